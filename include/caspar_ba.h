@@ -1,0 +1,178 @@
+/* caspar_ba.h — C ABI of the B200 (sm_100a) bundle-adjustment hot path.
+ *
+ * One Levenberg-Marquardt iteration on a reprojection-error problem, after the generated
+ * bundle-adjustment solver of "Caspar" (arxiv 2605.30583; /root/reference/PAPER.md):
+ *   - residual of the Snavely reprojection factor, PAPER.md:182-204 (section VI-A):
+ *       P = R(w) X + t,  p = -P_xy / P_z,  r = 1 + k1 |p|^2 + k2 |p|^4,  residual = f r p - pixel;
+ *   - Levenberg-Marquardt with quality-based damping (Madsen et al.), PAPER.md:163 (section V);
+ *   - preconditioned conjugate gradients with a block-Jacobi preconditioner, one block per node,
+ *     applied matrix-free from per-observation Jacobians, PAPER.md:163,167-169;
+ *   - one device memory block with views.
+ * BASELINE.json `north_star` fixes the variant built here: the linear system is the
+ * point-eliminated (Schur-complement) one, S = U' - W V'^-1 W^T, cameras are 9-vectors
+ * (angle-axis w, translation t, f, k1, k2) updated additively.  DESIGN.md lists every reading.
+ *
+ * Conventions
+ *   - Plain C, no exceptions cross the boundary.  Every call returns CASPAR_BA_OK (0) or a negative
+ *     CASPAR_BA_E* code; caspar_ba_last_error() gives the text of the last failure on a handle.
+ *   - "DEVICE" pointers are CUDA device pointers on the current device ("DEVICE or HOST" pointers are
+ *     read with cudaMemcpyDefault, so either works).  "HOST" pointers are ordinary host memory.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the default stream).  All work is
+ *     enqueued on it.  Calls that return host scalars synchronise that stream once before returning.
+ *   - The library owns ONE device arena allocated in caspar_ba_create and freed in caspar_ba_destroy.
+ *     Parameter arrays are BORROWED for the handle's lifetime and written only by an accepted
+ *     caspar_ba_lm_step (or caspar_ba_solve / caspar_ba_set_parameters_host).
+ *   - There is no CPU fallback: every step runs in the library's sm_100a kernels.
+ *   - Not thread-safe per handle; distinct handles are independent.
+ *
+ * Layouts: cameras [num_cameras][9] row-major float32 = w0 w1 w2 t0 t1 t2 f k1 k2;
+ * points [num_points][3] float32; observations [N][2] float32 pixels; indices int32.
+ */
+#ifndef CASPAR_BA_H
+#define CASPAR_BA_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CASPAR_BA_OK 0
+#define CASPAR_BA_EINVAL (-1)   /* null / negative sizes, index out of range, unsupported shape          */
+#define CASPAR_BA_ECUDA (-2)    /* a CUDA runtime call failed (text in caspar_ba_last_error)             */
+#define CASPAR_BA_ENOMEM (-3)   /* host or device allocation failed                                      */
+#define CASPAR_BA_ENUMERIC (-4) /* non-finite cost, non-positive pivot in a 3x3 / 9x9 block, p.Sp <= 0   */
+#define CASPAR_BA_ESTATE (-5)   /* call order, e.g. pcg_solve before linearize                           */
+
+#define CASPAR_BA_MAX_TRACK 1024 /* longest supported track (observations of one point) */
+
+typedef struct caspar_ba caspar_ba_t; /* opaque handle */
+
+typedef struct {
+  int32_t num_cameras, num_points;
+  int64_t num_observations;
+  float* cameras;              /* DEVICE [num_cameras][9]. Borrowed; updated in place by an accepted step. */
+  float* points;               /* DEVICE [num_points][3].  Borrowed; updated in place by an accepted step. */
+  const float* observations;   /* DEVICE or HOST [N][2] pixels.              Copied (reordered) at create. */
+  const int32_t* camera_index; /* DEVICE or HOST [N], 0 <= v < num_cameras.  Copied at create.             */
+  const int32_t* point_index;  /* DEVICE or HOST [N], 0 <= v < num_points.   Copied at create.             */
+  int32_t robust_loss;         /* 0 = none (F = 1/2 sum |r|^2), 1 = Cauchy (F = 1/2 sum c^2 log(1+|r|^2/c^2)) */
+  float robust_scale;          /* c in pixels (> 0 when robust_loss = 1)                                   */
+  int32_t damping_mode;        /* 0 = lambda * max(diag(J^T J), 1e-6) (Marquardt scaling), 1 = lambda * I  */
+} caspar_ba_problem;
+
+typedef struct {
+  int32_t iterations;  /* Schur matvecs performed                                 */
+  int32_t converged;   /* 1 iff |r_k| <= rel_tol |b| was reached                  */
+  double rel_residual; /* |r_k| / |b| of the recursive residual at exit           */
+  double rz0, rz;      /* r.M^-1 r at start and at exit                           */
+} caspar_ba_pcg_info;
+
+typedef struct {
+  double cost_before, cost_after; /* F at the current and at the trial parameters      */
+  double model_decrease;          /* L(0) - L(delta) = -delta.g - 1/2 |J delta|^2      */
+  double rho;                     /* gain ratio (cost_before - cost_after) / model_decrease */
+  int32_t accepted;
+  caspar_ba_pcg_info pcg;
+} caspar_ba_step_info;
+
+/* Build a solver for one problem: validates the indices, reorders the observations (sorted by point
+ * into tiles of whole points, camera runs contiguous inside a tile), carves the arena.
+ * Errors: EINVAL (bad sizes / indices / a track longer than CASPAR_BA_MAX_TRACK), ENOMEM, ECUDA. */
+int caspar_ba_create(const caspar_ba_problem* problem, void* cuda_stream, caspar_ba_t** out);
+
+/* Steps S1-S4: read the caller's parameter arrays, evaluate residuals and Jacobians of every
+ * observation, assemble the 9x9 camera and 3x3 point blocks and the gradient; cache them in the arena.
+ * cost_out: HOST, nullable; F at the current parameters.  Errors: ENUMERIC (non-finite cost), ECUDA. */
+int caspar_ba_linearize(caspar_ba_t* h, void* cuda_stream, double* cost_out);
+
+/* Steps S5-S8: solve (J^T J + lambda D) delta = -g through the Schur complement with block-Jacobi PCG,
+ * x0 = 0, stop when |r_k| <= rel_tol |b| or after max_iter matvecs; back-substitute the point steps.
+ * Leaves delta in the arena.  info: HOST, nullable.  Errors: ESTATE (no cached linearization),
+ * ENUMERIC (block not positive definite, p.Sp <= 0; delta then holds the last good iterate). */
+int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, void* cuda_stream,
+                        caspar_ba_pcg_info* info);
+
+/* Steps S1-S10: linearize if the cache is stale, pcg_solve, evaluate the trial point x + delta, gain ratio,
+ * then commit (parameters updated in place, cache stale) or discard (cache stays valid).
+ * accept_mode: 0 = accept iff rho > 0 and the trial cost is finite, 1 = always, 2 = never (dry run).
+ * info: HOST, required. */
+int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, int32_t accept_mode,
+                      void* cuda_stream, caspar_ba_step_info* info);
+
+/* `iterations` adaptive LM steps from lambda0 with Nielsen's damping update (accepted: lambda *=
+ * max(1/3, 1 - (2 rho - 1)^3), nu = 2; rejected: lambda *= nu, nu *= 2).  infos[iterations] and
+ * lambdas[iterations] (HOST, nullable) receive each step's record and the lambda it was solved with. */
+int caspar_ba_solve(caspar_ba_t* h, int32_t iterations, float lambda0, float rel_tol, int32_t max_iter,
+                    void* cuda_stream, caspar_ba_step_info* infos, float* lambdas);
+
+/* Step S9 without the update: F at the caller's current parameters.  cost_out: HOST, required. */
+int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out);
+
+void caspar_ba_destroy(caspar_ba_t* h);
+
+/* Host-buffer convenience (end-to-end path): copy HOST parameter arrays ([Nc][9], [Np][3]; pinned memory
+ * makes the copy asynchronous) into the borrowed device arrays and mark the cache stale / copy the
+ * device arrays back to HOST buffers.  get synchronises the stream. */
+int caspar_ba_set_parameters_host(caspar_ba_t* h, const float* cameras_host, const float* points_host,
+                                  void* cuda_stream);
+int caspar_ba_get_parameters_host(caspar_ba_t* h, float* cameras_host, float* points_host, void* cuda_stream);
+
+/* ---- test-only exports: slow path, caller's observation / node order, array-of-structs float64 ---- */
+enum {
+  CASPAR_BA_RESIDUALS = 0, /* [N][2]          (robust-reweighted if enabled)   */
+  CASPAR_BA_JC = 1,        /* [N][2][9]                                          */
+  CASPAR_BA_JP = 2,        /* [N][2][3]                                          */
+  CASPAR_BA_U = 3,         /* [Nc][9][9]                                         */
+  CASPAR_BA_V = 4,         /* [Np][3][3]                                         */
+  CASPAR_BA_G = 5,         /* [9 Nc + 3 Np]                                      */
+  CASPAR_BA_SCHUR_RHS = 6, /* [9 Nc]        (after pcg_solve)                    */
+  CASPAR_BA_DELTA = 7      /* [9 Nc + 3 Np] (after pcg_solve)                    */
+};
+/* device_dst: DEVICE double array with exactly `count` elements of the shape above. */
+int caspar_ba_export(caspar_ba_t* h, int32_t what, double* device_dst, size_t count, void* cuda_stream);
+/* q = S p at damping lambda from the cached linearization; p_dev, q_dev: DEVICE double [9 Nc]. */
+int caspar_ba_schur_matvec(caspar_ba_t* h, float lambda, const double* p_dev, double* q_dev, void* cuda_stream);
+
+/* ---- introspection ---- */
+typedef struct {
+  int32_t tile_slots;        /* T: observation slots (= threads) per tile                       */
+  int32_t num_tiles;
+  int64_t padded_slots;      /* num_tiles * T                                                   */
+  int64_t camera_runs;       /* sum over tiles of distinct cameras in the tile                  */
+  int64_t arena_bytes;
+  int64_t kernels_launched;  /* kernels this handle has launched since create (or reset)         */
+  /* CUDA-event time of the two dominant kernels, accumulated while profiling is on:              */
+  double linearize_ms_total, matvec_ms_total;
+  int64_t linearize_count, matvec_count;
+} caspar_ba_stats;
+/* Synchronises the stream the timed kernels ran on, then fills *out. */
+int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out);
+/* enable != 0: bracket every linearize and Schur-matvec kernel with CUDA events on its stream.
+ * Also resets the accumulated times and the launch counter. */
+int caspar_ba_set_profiling(caspar_ba_t* h, int32_t enable);
+/* ---- step S0 on its own (host only, no CUDA call): the observation reordering that create performs ----
+ * cam_index / point_index: HOST [n].  tile = 0 lets the library choose T, else 256 | 512 | 1024.
+ * caspar_ba_layout_copy copies one of the planned arrays to HOST memory (`bytes` must match exactly):
+ *   0 obs_of_slot int32[slots]   1 cam int32[slots]        2 rank uint16[slots]     3 tile_pt int32[tiles+1]
+ *   4 run_begin int32[tiles+1]   5 run_cam int32[runs+tiles+1]  6 run_slot uint16[runs+tiles+1]
+ *   7 pt_ptr int32[np_obs+1]     8 pt_perm int32[np]       9 cslot int32[n]         10 chunk_cam int32[chunks]
+ *   11 chunk_begin int32[chunks+1] */
+typedef struct caspar_ba_layout caspar_ba_layout_t;
+typedef struct {
+  int32_t tile_slots, num_tiles, observed_points, num_chunks;
+  int64_t padded_slots, camera_runs;
+} caspar_ba_layout_info;
+int caspar_ba_layout_create(int32_t num_cameras, int32_t num_points, int64_t n, const int32_t* cam_index,
+                            const int32_t* point_index, int32_t tile, caspar_ba_layout_t** out);
+int caspar_ba_layout_get_info(const caspar_ba_layout_t* l, caspar_ba_layout_info* info);
+int caspar_ba_layout_copy(const caspar_ba_layout_t* l, int32_t which, void* dst_host, size_t bytes);
+void caspar_ba_layout_destroy(caspar_ba_layout_t* l);
+
+/* Valid until the next call on the handle; never NULL. */
+const char* caspar_ba_last_error(const caspar_ba_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -140,8 +140,8 @@ class OracleBA:
                    scene.robust_scale if robust_scale is None else robust_scale, damping_mode)
 
     def close(self):
-        if getattr(self, "_h", None):
-            lib().oracle_ba_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:   # (_lib is gone at interpreter shutdown)
+            _lib.oracle_ba_destroy(self._h)
             self._h = None
 
     __del__ = close

@@ -1,0 +1,669 @@
+// ba_api.cu — the C ABI of include/caspar_ba.h: arena, state machine, PCG loop, LM step.
+// Host code only orchestrates launches and reads back a handful of scalars per call; every step of
+// the path (S1-S9) runs in the kernels of ba_kernels.cu.  There is no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "ba_internal.h"
+
+namespace cba {
+long long take_launch_count();
+}
+
+using namespace cba;
+
+struct caspar_ba {
+  caspar_ba_problem pb{};
+  View v{};
+  void* arena = nullptr;
+  size_t arena_bytes = 0;
+  long long camera_runs = 0;
+  bool linearized = false;
+  bool have_delta = false;
+  double prepared_lambda = -1.0;
+  bool prepared = false;
+  double cost = 0.0;  // F at the cached linearization
+  std::string err;
+  long long launches = 0;
+  // pinned host mirrors of the device scalars
+  PcgScalars* h_pcg = nullptr;
+  StepScalars* h_step = nullptr;
+  int* h_flags = nullptr;  // done flags polled during a tolerance-driven PCG run
+  // profiling
+  bool profiling = false;
+  std::vector<cudaEvent_t> ev_lin, ev_mv;  // start/stop pairs awaiting readout
+  cudaStream_t prof_stream = nullptr;
+  double lin_ms = 0.0, mv_ms = 0.0;
+  long long lin_n = 0, mv_n = 0;
+  std::vector<cudaEvent_t> ev_pool;
+  cudaEvent_t poll_ev[2] = {nullptr, nullptr};
+};
+
+namespace {
+
+int fail(caspar_ba* h, int code, const std::string& msg) {
+  if (h) h->err = msg;
+  return code;
+}
+
+int cuda_fail(caspar_ba* h, cudaError_t e, const char* where) {
+  return fail(h, e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA,
+              std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+#define CK(call)                                              \
+  do {                                                        \
+    cudaError_t e_ = (call);                                  \
+    if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);    \
+  } while (0)
+
+// bump allocator over the arena ("a single block of GPU memory ... all utilized arrays are views")
+struct Carver {
+  char* base;
+  size_t off = 0;
+  explicit Carver(void* b) : base((char*)b) {}
+  template <class T>
+  T* take(size_t count) {
+    off = (off + 255) & ~size_t(255);
+    T* p = base ? (T*)(base + off) : nullptr;
+    off += (count ? count : 1) * sizeof(T);
+    return p;
+  }
+};
+
+// One pass lays out the views; called with base = nullptr to size the arena, then with the real base.
+size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
+  View& v = h->v;
+  Carver c(base);
+  const size_t S = (size_t)v.n_slots, NC = (size_t)v.nc, NP = (size_t)v.np;
+  for (int i = 0; i < 6; ++i) v.J[i] = c.take<float4>(S);
+  v.res = c.take<float2>(S);
+  v.px = c.take<float2>(S);
+  v.cam = c.take<int>(S);
+  v.obs_of_slot = c.take<int>(S);
+  v.rank = c.take<unsigned short>(S);
+  v.tile_pt = c.take<int>(ro.tile_pt.size());
+  v.run_begin = c.take<int>(ro.run_begin.size());
+  v.run_cam = c.take<int>(ro.run_cam.size());
+  v.run_slot = c.take<unsigned short>(ro.run_slot.size());
+  v.pt_ptr = c.take<int>(ro.pt_ptr.size());
+  v.pt_perm = c.take<int>(NP);
+  v.cslot = c.take<int>(ro.cslot.size());
+  v.chunk_cam = c.take<int>(ro.chunk_cam.size());
+  v.chunk_begin = c.take<int>(ro.chunk_begin.size());
+  v.pts = c.take<float4>(NP);
+  v.pts_trial = c.take<float4>(NP);
+  v.V0 = c.take<float4>(NP);
+  v.V1 = c.take<float2>(NP);
+  v.gp = c.take<float4>(NP);
+  v.Vinv0 = c.take<float4>(NP);
+  v.Vinv1 = c.take<float2>(NP);
+  v.dp = c.take<float4>(NP);
+  v.cams_trial = c.take<float>(9 * NC);
+  v.cam_table = c.take<float>(kCamTableFloats * NC);
+  v.cam_table_trial = c.take<float>(kCamTableFloats * NC);
+  v.Ug = c.take<double>(kUg * NC);
+  v.Minv = c.take<double>(81 * NC);
+  v.lamD = c.take<double>(9 * NC);
+  v.b = c.take<double>(9 * NC);
+  v.x = c.take<double>(9 * NC);
+  v.r = c.take<double>(9 * NC);
+  v.z = c.take<double>(9 * NC);
+  v.p = c.take<double>(9 * NC);
+  v.q = c.take<double>(9 * NC);
+  v.p32 = c.take<float>(kCamPad * NC);
+  v.pcg = c.take<PcgScalars>(1);
+  v.step = c.take<StepScalars>(1);
+  return (c.off + 255) & ~size_t(255);
+}
+
+template <class T>
+cudaError_t upload(const void* dst, const std::vector<T>& src, cudaStream_t s) {
+  if (src.empty()) return cudaSuccess;
+  return cudaMemcpyAsync(const_cast<void*>(dst), src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+}
+
+void account(caspar_ba* h) { h->launches += take_launch_count(); }
+
+cudaEvent_t get_event(caspar_ba* h) {
+  if (!h->ev_pool.empty()) {
+    cudaEvent_t e = h->ev_pool.back();
+    h->ev_pool.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+
+// Fold finished event pairs into the totals (the caller has synchronised the stream).
+void drain_events(caspar_ba* h) {
+  auto fold = [&](std::vector<cudaEvent_t>& evs, double& ms, long long& n) {
+    for (size_t i = 0; i + 1 < evs.size(); i += 2) {
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, evs[i], evs[i + 1]) == cudaSuccess) {
+        ms += t;
+        n += 1;
+      }
+      h->ev_pool.push_back(evs[i]);
+      h->ev_pool.push_back(evs[i + 1]);
+    }
+    evs.clear();
+  };
+  fold(h->ev_lin, h->lin_ms, h->lin_n);
+  fold(h->ev_mv, h->mv_ms, h->mv_n);
+}
+
+struct Timed {  // brackets one kernel launch with events when profiling is on
+  caspar_ba* h;
+  std::vector<cudaEvent_t>* evs;
+  cudaStream_t s;
+  Timed(caspar_ba* h_, std::vector<cudaEvent_t>* e, cudaStream_t s_) : h(h_), evs(e), s(s_) {
+    if (h->profiling) {
+      cudaEvent_t a = get_event(h);
+      cudaEventRecord(a, s);
+      evs->push_back(a);
+      h->prof_stream = s;
+    }
+  }
+  ~Timed() {
+    if (h->profiling) {
+      cudaEvent_t b = get_event(h);
+      cudaEventRecord(b, s);
+      evs->push_back(b);
+    }
+  }
+};
+
+int sync_step_scalars(caspar_ba* h, cudaStream_t s) {
+  CK(cudaMemcpyAsync(h->h_step, h->v.step, sizeof(StepScalars), cudaMemcpyDeviceToHost, s));
+  CK(cudaMemcpyAsync(h->h_pcg, h->v.pcg, sizeof(PcgScalars), cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  if (h->profiling) drain_events(h);
+  return 0;
+}
+
+int do_linearize(caspar_ba* h, cudaStream_t s) {
+  View& v = h->v;
+  CK(cudaMemsetAsync(v.step, 0, sizeof(StepScalars), s));
+  CK(cudaMemsetAsync(v.Ug, 0, sizeof(double) * kUg * (size_t)(v.nc ? v.nc : 1), s));
+  CK(launch_pack_points(v, v.points, v.pts, s));
+  CK(launch_camera_prepass(v, v.cameras, v.cam_table, s));
+  {
+    Timed t(h, &h->ev_lin, s);
+    CK(launch_linearize(v, s));
+  }
+  CK(launch_assemble_cameras(v, s));
+  account(h);
+  h->linearized = true;
+  h->prepared = false;
+  h->have_delta = false;
+  return 0;
+}
+
+int do_prepare(caspar_ba* h, double lambda, cudaStream_t s) {
+  if (h->prepared && h->prepared_lambda == lambda) return 0;
+  CK(launch_prepare_blocks(h->v, lambda, s));
+  account(h);
+  h->prepared = true;
+  h->prepared_lambda = lambda;
+  return 0;
+}
+
+// Enqueue S5-S8.  No host synchronisation unless rel_tol > 0, where the device-side `done` flag is
+// polled one chunk behind the launches so that the GPU never waits for the host.
+int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream_t s) {
+  View& v = h->v;
+  h->prepared = false;  // the right-hand side b is rebuilt by prepare (it starts from -g_c)
+  CK(cudaMemsetAsync(&v.step->jd2, 0, 2 * sizeof(double) + 2 * sizeof(int), s));  // jd2, dg, bad_block
+  int rc = do_prepare(h, lambda, s);
+  if (rc) return rc;
+  CK(cudaMemsetAsync(v.pcg, 0, sizeof(PcgScalars), s));
+  CK(launch_schur_rhs(v, s));
+  CK(launch_pcg_init(v, s));
+  const double tol2 = rel_tol * rel_tol;
+  const int chunk = 8;
+  int polled = 0;  // chunks whose flag copy has been enqueued
+  bool stop = false;
+  for (int it = 0; it < max_iter && !stop; ++it) {
+    {
+      Timed t(h, &h->ev_mv, s);
+      CK(launch_schur_matvec(v, it, s));
+    }
+    CK(launch_pcg_update(v, it, tol2, s));
+    if (rel_tol > 0.0 && (it + 1) % chunk == 0 && it + 1 < max_iter) {
+      const int slot = polled & 1;
+      if (polled >= 2) {  // wait for the copy enqueued two chunks ago (slot reuse) and look at it
+        CK(cudaEventSynchronize(h->poll_ev[slot]));
+        if (h->h_flags[slot]) stop = true;
+      }
+      if (!stop) {
+        CK(cudaMemcpyAsync(&h->h_flags[slot], &v.pcg->done, sizeof(int), cudaMemcpyDeviceToHost, s));
+        CK(cudaEventRecord(h->poll_ev[slot], s));
+        ++polled;
+      }
+    }
+  }
+  CK(launch_backsub(v, s));
+  account(h);
+  h->have_delta = true;
+  return 0;
+}
+
+void fill_pcg_info(const caspar_ba* h, caspar_ba_pcg_info* info) {
+  const PcgScalars& p = *h->h_pcg;
+  info->iterations = p.iters;
+  info->converged = p.converged;
+  info->rel_residual = p.bnorm2 > 0.0 ? std::sqrt(p.rr / p.bnorm2) : 0.0;
+  info->rz0 = p.iters > 0 ? p.rz0 : p.rz[0];
+  info->rz = p.rz[p.iters & 1];
+}
+
+int check_numeric(caspar_ba* h) {
+  if (h->h_step->bad_block) return fail(h, CASPAR_BA_ENUMERIC, "a damped 9x9 or 3x3 block is not positive definite");
+  if (h->h_pcg->breakdown) return fail(h, CASPAR_BA_ENUMERIC, "PCG breakdown: p.Sp <= 0 or not finite");
+  return 0;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t** out) {
+  if (!pb || !out) return CASPAR_BA_EINVAL;
+  *out = nullptr;
+  if (pb->num_cameras < 0 || pb->num_points < 0 || pb->num_observations < 0) return CASPAR_BA_EINVAL;
+  if (pb->num_observations > 0 && (!pb->observations || !pb->camera_index || !pb->point_index)) return CASPAR_BA_EINVAL;
+  if ((pb->num_cameras > 0 && !pb->cameras) || (pb->num_points > 0 && !pb->points)) return CASPAR_BA_EINVAL;
+  if (pb->robust_loss != 0 && pb->robust_loss != 1) return CASPAR_BA_EINVAL;
+  if (pb->robust_loss == 1 && !(pb->robust_scale > 0.f)) return CASPAR_BA_EINVAL;
+  if (pb->damping_mode != 0 && pb->damping_mode != 1) return CASPAR_BA_EINVAL;
+  if (pb->num_observations > 0 && (pb->num_cameras == 0 || pb->num_points == 0)) return CASPAR_BA_EINVAL;
+  caspar_ba* h = new (std::nothrow) caspar_ba();
+  if (!h) return CASPAR_BA_ENOMEM;
+  h->pb = *pb;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const long long n = pb->num_observations;
+  auto bail = [&](int code) {
+    caspar_ba_destroy(h);
+    return code;
+  };
+  // indices to the host (the source may be device or host memory)
+  std::vector<int> cam_idx((size_t)n), pt_idx((size_t)n);
+  if (n > 0) {
+    cudaError_t e = cudaMemcpy(cam_idx.data(), pb->camera_index, sizeof(int) * (size_t)n, cudaMemcpyDefault);
+    if (e == cudaSuccess) e = cudaMemcpy(pt_idx.data(), pb->point_index, sizeof(int) * (size_t)n, cudaMemcpyDefault);
+    if (e != cudaSuccess) return bail(e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA);
+  }
+  int forced = 0;
+  if (const char* env = std::getenv("CASPAR_BA_TILE")) forced = std::atoi(env);
+  Reordered ro;
+  std::string err;
+  int rc = CASPAR_BA_OK;
+  try {
+    rc = reorder_observations(pb->num_cameras, pb->num_points, n, cam_idx.data(), pt_idx.data(), forced, &ro, &err);
+  } catch (const std::bad_alloc&) {
+    return bail(CASPAR_BA_ENOMEM);
+  }
+  if (rc) return bail(rc);
+  View& v = h->v;
+  v.nc = pb->num_cameras;
+  v.np = pb->num_points;
+  v.np_obs = ro.np_obs;
+  v.T = ro.T;
+  v.num_tiles = ro.num_tiles;
+  v.n_slots = ro.n_slots;
+  v.num_chunks = (int)ro.chunk_cam.size();
+  v.robust = pb->robust_loss;
+  v.robust_c2 = pb->robust_scale * pb->robust_scale;
+  v.damping_mode = pb->damping_mode;
+  v.cameras = pb->cameras;
+  v.points = pb->points;
+  h->camera_runs = ro.camera_runs;
+  h->arena_bytes = carve(h, nullptr, ro);
+  cudaError_t e = cudaMalloc(&h->arena, h->arena_bytes);
+  if (e != cudaSuccess) return bail(CASPAR_BA_ENOMEM);
+  carve(h, h->arena, ro);
+  e = cudaMemsetAsync(h->arena, 0, h->arena_bytes, s);
+  if (e == cudaSuccess) e = upload(v.cam, ro.cam, s);
+  if (e == cudaSuccess) e = upload(v.obs_of_slot, ro.obs_of_slot, s);
+  if (e == cudaSuccess) e = upload(v.rank, ro.rank, s);
+  if (e == cudaSuccess) e = upload(v.tile_pt, ro.tile_pt, s);
+  if (e == cudaSuccess) e = upload(v.run_begin, ro.run_begin, s);
+  if (e == cudaSuccess) e = upload(v.run_cam, ro.run_cam, s);
+  if (e == cudaSuccess) e = upload(v.run_slot, ro.run_slot, s);
+  if (e == cudaSuccess) e = upload(v.pt_ptr, ro.pt_ptr, s);
+  if (e == cudaSuccess) e = upload(v.pt_perm, ro.pt_perm, s);
+  if (e == cudaSuccess) e = upload(v.cslot, ro.cslot, s);
+  if (e == cudaSuccess) e = upload(v.chunk_cam, ro.chunk_cam, s);
+  if (e == cudaSuccess) e = upload(v.chunk_begin, ro.chunk_begin, s);
+  // pixels: the caller's array may live on either side; stage through the device if it is host memory
+  float* obs_dev = nullptr;
+  if (e == cudaSuccess && n > 0) {
+    cudaPointerAttributes attr{};
+    bool on_device = cudaPointerGetAttributes(&attr, pb->observations) == cudaSuccess &&
+                     (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged);
+    cudaGetLastError();
+    const float* src = pb->observations;
+    if (!on_device) {
+      e = cudaMalloc(&obs_dev, sizeof(float) * 2 * (size_t)n);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(obs_dev, pb->observations, sizeof(float) * 2 * (size_t)n, cudaMemcpyDefault, s);
+      src = obs_dev;
+    }
+    if (e == cudaSuccess) e = launch_gather_observations(v, src, const_cast<float2*>(v.px), s);
+  }
+  if (e == cudaSuccess) e = cudaMallocHost(&h->h_pcg, sizeof(PcgScalars));
+  if (e == cudaSuccess) e = cudaMallocHost(&h->h_step, sizeof(StepScalars));
+  if (e == cudaSuccess) e = cudaMallocHost(&h->h_flags, 2 * sizeof(int));
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->poll_ev[0], cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->poll_ev[1], cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);  // the host vectors above die with this scope
+  if (obs_dev) cudaFree(obs_dev);
+  account(h);
+  if (e != cudaSuccess) return bail(e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA);
+  *out = h;
+  return CASPAR_BA_OK;
+}
+
+void caspar_ba_destroy(caspar_ba_t* h) {
+  if (!h) return;
+  for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+  for (cudaEvent_t e : h->ev_lin) cudaEventDestroy(e);
+  for (cudaEvent_t e : h->ev_mv) cudaEventDestroy(e);
+  for (cudaEvent_t e : h->poll_ev)
+    if (e) cudaEventDestroy(e);
+  if (h->h_pcg) cudaFreeHost(h->h_pcg);
+  if (h->h_step) cudaFreeHost(h->h_step);
+  if (h->h_flags) cudaFreeHost(h->h_flags);
+  if (h->arena) cudaFree(h->arena);
+  delete h;
+}
+
+int caspar_ba_linearize(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
+  if (!h) return CASPAR_BA_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int rc = do_linearize(h, s);
+  if (rc) return rc;
+  rc = sync_step_scalars(h, s);
+  if (rc) return rc;
+  h->cost = 0.5 * h->h_step->cost;
+  if (cost_out) *cost_out = h->cost;
+  if (!std::isfinite(h->cost)) {
+    h->linearized = false;
+    return fail(h, CASPAR_BA_ENUMERIC, "non-finite cost");
+  }
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
+  if (!h || !cost_out) return CASPAR_BA_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  View& v = h->v;
+  // evaluated in the trial buffers so that a cached linearization stays untouched
+  CK(cudaMemsetAsync(&v.step->trial_cost, 0, sizeof(double), s));
+  CK(launch_pack_points(v, v.points, v.pts_trial, s));
+  CK(launch_camera_prepass(v, v.cameras, v.cam_table_trial, s));
+  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
+  account(h);
+  int rc = sync_step_scalars(h, s);
+  if (rc) return rc;
+  *cost_out = 0.5 * h->h_step->trial_cost;
+  return std::isfinite(*cost_out) ? CASPAR_BA_OK : fail(h, CASPAR_BA_ENUMERIC, "non-finite cost");
+}
+
+int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, void* cuda_stream,
+                        caspar_ba_pcg_info* info) {
+  if (!h || max_iter < 0 || !(lambda >= 0.f) || !(rel_tol >= 0.f)) return CASPAR_BA_EINVAL;
+  if (!h->linearized) return fail(h, CASPAR_BA_ESTATE, "pcg_solve before linearize");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int rc = do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
+  if (rc) return rc;
+  rc = sync_step_scalars(h, s);
+  if (rc) return rc;
+  if (info) fill_pcg_info(h, info);
+  return check_numeric(h);
+}
+
+int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, int32_t accept_mode,
+                      void* cuda_stream, caspar_ba_step_info* info) {
+  if (!h || !info || max_iter < 0 || accept_mode < 0 || accept_mode > 2 || !(lambda >= 0.f) || !(rel_tol >= 0.f))
+    return CASPAR_BA_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  View& v = h->v;
+  std::memset(info, 0, sizeof *info);
+  int rc;
+  const bool fresh = !h->linearized;
+  if (fresh) {
+    rc = do_linearize(h, s);
+    if (rc) return rc;
+  }
+  rc = do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
+  if (rc) return rc;
+  // trial point and its cost (S9)
+  CK(cudaMemsetAsync(&v.step->trial_cost, 0, sizeof(double), s));
+  CK(launch_trial_update(v, s));
+  CK(launch_camera_prepass(v, v.cams_trial, v.cam_table_trial, s));
+  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
+  account(h);
+  rc = sync_step_scalars(h, s);  // the one host synchronisation of the step
+  if (rc) return rc;
+  if (fresh) h->cost = 0.5 * h->h_step->cost;
+  if (!std::isfinite(h->cost)) {
+    h->linearized = false;
+    return fail(h, CASPAR_BA_ENUMERIC, "non-finite cost");
+  }
+  fill_pcg_info(h, &info->pcg);
+  rc = check_numeric(h);
+  if (rc) return rc;
+  // S10 gain ratio (host scalars)
+  info->cost_before = h->cost;
+  info->cost_after = 0.5 * h->h_step->trial_cost;
+  info->model_decrease = -h->h_step->dg - 0.5 * h->h_step->jd2;
+  info->rho = (info->cost_before - info->cost_after) / info->model_decrease;
+  bool accept;
+  if (accept_mode == 1) accept = true;
+  else if (accept_mode == 2) accept = false;
+  else accept = std::isfinite(info->cost_after) && info->rho > 0.0;
+  info->accepted = accept ? 1 : 0;
+  if (accept) {
+    CK(launch_commit(v, s));
+    account(h);
+    h->linearized = false;
+    h->prepared = false;
+  }
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_solve(caspar_ba_t* h, int32_t iterations, float lambda0, float rel_tol, int32_t max_iter,
+                    void* cuda_stream, caspar_ba_step_info* infos, float* lambdas) {
+  if (!h || iterations < 0) return CASPAR_BA_EINVAL;
+  double lambda = lambda0, nu = 2.0;
+  for (int it = 0; it < iterations; ++it) {
+    caspar_ba_step_info info;
+    if (lambdas) lambdas[it] = (float)lambda;
+    int rc = caspar_ba_lm_step(h, (float)lambda, rel_tol, max_iter, 0, cuda_stream, &info);
+    if (rc) return rc;
+    if (infos) infos[it] = info;
+    if (info.accepted) {  // Nielsen's update (Madsen, Nielsen, Tingleff 2004, eq. 3.16 / PAPER.md:163)
+      const double c = 2.0 * info.rho - 1.0;
+      lambda *= std::fmax(1.0 / 3.0, 1.0 - c * c * c);
+      nu = 2.0;
+    } else {
+      lambda *= nu;
+      nu *= 2.0;
+    }
+  }
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_set_parameters_host(caspar_ba_t* h, const float* cameras_host, const float* points_host,
+                                  void* cuda_stream) {
+  if (!h || (h->v.nc > 0 && !cameras_host) || (h->v.np > 0 && !points_host)) return CASPAR_BA_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (h->v.nc > 0)
+    CK(cudaMemcpyAsync(h->v.cameras, cameras_host, sizeof(float) * 9 * (size_t)h->v.nc, cudaMemcpyHostToDevice, s));
+  if (h->v.np > 0)
+    CK(cudaMemcpyAsync(h->v.points, points_host, sizeof(float) * 3 * (size_t)h->v.np, cudaMemcpyHostToDevice, s));
+  h->linearized = false;
+  h->prepared = false;
+  h->have_delta = false;
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_get_parameters_host(caspar_ba_t* h, float* cameras_host, float* points_host, void* cuda_stream) {
+  if (!h || (h->v.nc > 0 && !cameras_host) || (h->v.np > 0 && !points_host)) return CASPAR_BA_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (h->v.nc > 0)
+    CK(cudaMemcpyAsync(cameras_host, h->v.cameras, sizeof(float) * 9 * (size_t)h->v.nc, cudaMemcpyDeviceToHost, s));
+  if (h->v.np > 0)
+    CK(cudaMemcpyAsync(points_host, h->v.points, sizeof(float) * 3 * (size_t)h->v.np, cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_export(caspar_ba_t* h, int32_t what, double* device_dst, size_t count, void* cuda_stream) {
+  if (!h || !device_dst) return CASPAR_BA_EINVAL;
+  const size_t N = (size_t)h->pb.num_observations, nc = (size_t)h->v.nc, np = (size_t)h->v.np;
+  size_t need = 0;
+  switch (what) {
+    case CASPAR_BA_RESIDUALS: need = 2 * N; break;
+    case CASPAR_BA_JC: need = 18 * N; break;
+    case CASPAR_BA_JP: need = 6 * N; break;
+    case CASPAR_BA_U: need = 81 * nc; break;
+    case CASPAR_BA_V: need = 9 * np; break;
+    case CASPAR_BA_G: case CASPAR_BA_DELTA: need = 9 * nc + 3 * np; break;
+    case CASPAR_BA_SCHUR_RHS: need = 9 * nc; break;
+    default: return fail(h, CASPAR_BA_EINVAL, "unknown export id");
+  }
+  if (count != need) return fail(h, CASPAR_BA_EINVAL, "export: wrong element count");
+  const bool solve_product = what == CASPAR_BA_SCHUR_RHS || what == CASPAR_BA_DELTA;
+  if (solve_product ? !h->have_delta : !h->linearized) return fail(h, CASPAR_BA_ESTATE, "export: nothing cached");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  CK(launch_export(h->v, what, device_dst, s));
+  account(h);
+  CK(cudaStreamSynchronize(s));
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_schur_matvec(caspar_ba_t* h, float lambda, const double* p_dev, double* q_dev, void* cuda_stream) {
+  if (!h || !p_dev || !q_dev || !(lambda >= 0.f)) return CASPAR_BA_EINVAL;
+  if (!h->linearized) return fail(h, CASPAR_BA_ESTATE, "schur_matvec before linearize");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int rc = do_prepare(h, (double)lambda, s);
+  if (rc) return rc;
+  CK(cudaMemsetAsync(h->v.pcg, 0, sizeof(PcgScalars), s));
+  {
+    Timed t(h, &h->ev_mv, s);  // brackets load + pass + finish; the pass dominates
+    CK(launch_matvec_standalone(h->v, p_dev, q_dev, s));
+  }
+  account(h);
+  h->have_delta = false;  // x / p buffers were reused
+  rc = sync_step_scalars(h, s);
+  if (rc) return rc;
+  return check_numeric(h);
+}
+
+int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {
+  if (!h || !out) return CASPAR_BA_EINVAL;
+  if (h->profiling && (!h->ev_lin.empty() || !h->ev_mv.empty())) {
+    CK(cudaStreamSynchronize(h->prof_stream));
+    drain_events(h);
+  }
+  out->tile_slots = h->v.T;
+  out->num_tiles = h->v.num_tiles;
+  out->padded_slots = h->v.n_slots;
+  out->camera_runs = h->camera_runs;
+  out->arena_bytes = (int64_t)h->arena_bytes;
+  out->kernels_launched = h->launches;
+  out->linearize_ms_total = h->lin_ms;
+  out->matvec_ms_total = h->mv_ms;
+  out->linearize_count = h->lin_n;
+  out->matvec_count = h->mv_n;
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_set_profiling(caspar_ba_t* h, int32_t enable) {
+  if (!h) return CASPAR_BA_EINVAL;
+  if (h->prof_stream || !h->ev_lin.empty() || !h->ev_mv.empty()) {
+    cudaStreamSynchronize(h->prof_stream);
+    drain_events(h);
+  }
+  h->profiling = enable != 0;
+  h->lin_ms = h->mv_ms = 0.0;
+  h->lin_n = h->mv_n = 0;
+  h->launches = 0;
+  return CASPAR_BA_OK;
+}
+
+const char* caspar_ba_last_error(const caspar_ba_t* h) { return h ? h->err.c_str() : "null handle"; }
+
+// ---- S0 on its own (host only) ------------------------------------------------------------------
+struct caspar_ba_layout {
+  Reordered ro;
+};
+
+int caspar_ba_layout_create(int32_t nc, int32_t np, int64_t n, const int32_t* cam_index, const int32_t* point_index,
+                            int32_t tile, caspar_ba_layout_t** out) {
+  if (!out || nc < 0 || np < 0 || n < 0 || (n > 0 && (!cam_index || !point_index))) return CASPAR_BA_EINVAL;
+  caspar_ba_layout* l = new (std::nothrow) caspar_ba_layout();
+  if (!l) return CASPAR_BA_ENOMEM;
+  std::string err;
+  int rc;
+  try {
+    rc = reorder_observations(nc, np, n, cam_index, point_index, tile, &l->ro, &err);
+  } catch (const std::bad_alloc&) {
+    rc = CASPAR_BA_ENOMEM;
+  }
+  if (rc) {
+    delete l;
+    return rc;
+  }
+  *out = l;
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_layout_get_info(const caspar_ba_layout_t* l, caspar_ba_layout_info* info) {
+  if (!l || !info) return CASPAR_BA_EINVAL;
+  info->tile_slots = l->ro.T;
+  info->num_tiles = l->ro.num_tiles;
+  info->observed_points = l->ro.np_obs;
+  info->num_chunks = (int32_t)l->ro.chunk_cam.size();
+  info->padded_slots = l->ro.n_slots;
+  info->camera_runs = l->ro.camera_runs;
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_layout_copy(const caspar_ba_layout_t* l, int32_t which, void* dst, size_t bytes) {
+  if (!l || !dst) return CASPAR_BA_EINVAL;
+  const Reordered& r = l->ro;
+  const void* src = nullptr;
+  size_t have = 0;
+  const size_t slots = (size_t)r.n_slots;
+  auto pick = [&](const void* p, size_t n) { src = p; have = n; };
+  switch (which) {
+    case 0: pick(r.obs_of_slot.data(), slots * sizeof(int)); break;
+    case 1: pick(r.cam.data(), slots * sizeof(int)); break;
+    case 2: pick(r.rank.data(), slots * sizeof(unsigned short)); break;
+    case 3: pick(r.tile_pt.data(), r.tile_pt.size() * sizeof(int)); break;
+    case 4: pick(r.run_begin.data(), r.run_begin.size() * sizeof(int)); break;
+    case 5: pick(r.run_cam.data(), r.run_cam.size() * sizeof(int)); break;
+    case 6: pick(r.run_slot.data(), r.run_slot.size() * sizeof(unsigned short)); break;
+    case 7: pick(r.pt_ptr.data(), r.pt_ptr.size() * sizeof(int)); break;
+    case 8: pick(r.pt_perm.data(), r.pt_perm.size() * sizeof(int)); break;
+    case 9: pick(r.cslot.data(), (size_t)(r.pt_ptr.empty() ? 0 : r.pt_ptr.back()) * sizeof(int)); break;
+    case 10: pick(r.chunk_cam.data(), r.chunk_cam.size() * sizeof(int)); break;
+    case 11: pick(r.chunk_begin.data(), r.chunk_begin.size() * sizeof(int)); break;
+    default: return CASPAR_BA_EINVAL;
+  }
+  if (bytes != have) return CASPAR_BA_EINVAL;
+  if (have) std::memcpy(dst, src, have);
+  return CASPAR_BA_OK;
+}
+
+void caspar_ba_layout_destroy(caspar_ba_layout_t* l) { delete l; }
+
+}  // extern "C"

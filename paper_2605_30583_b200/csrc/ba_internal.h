@@ -1,0 +1,156 @@
+// ba_internal.h — internal layout of the B200 bundle-adjustment path (not part of the C ABI).
+//
+// Data layout in HBM:
+//   * Observations are permuted once at create (S0): points are ordered by their lowest camera id
+//     (camera locality per tile), packed greedily into TILES of whole points with T slots each
+//     (T = threads per block = 256 | 512 | 1024), and inside a tile the slots are sorted by camera so
+//     that equal-camera RUNS are contiguous.  Unused slots at the end of a tile are padding (cam = -1).
+//   * Per-slot arrays (length num_tiles * T, slot-major, so a warp reads 32 consecutive elements):
+//       px   float2   measured pixel
+//       cam  int32    camera id (-1 = padding)
+//       rank uint16   position of the slot's observation in the tile's POINT-major order
+//       J    6 x float4 chunk arrays: the 24 floats (J_c 2x9 row-major, then J_p 2x3 row-major) of one
+//                     observation, chunk c = floats [4c, 4c+4)  ("blocked struct of arrays")
+//       res  float2   residual (robust-reweighted)
+//   * Per-tile: first internal point, and a run table (camera id + first slot of each camera run).
+//   * Per-point arrays are in INTERNAL point order (pt_perm maps internal -> caller id).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/caspar_ba.h"
+
+namespace cba {
+
+constexpr int kCamTableFloats = 28;  // per-camera table row (7 x float4), see camera_prepass_kernel
+constexpr int kCamPad = 12;          // fp32 camera-vector copies (p, delta_c) are padded 9 -> 12 floats
+constexpr int kUg = 54;              // 45 upper-triangle entries of U_j + 9 of g_c,j, fp64 accumulators
+constexpr int kChunkSlots = 1024;    // camera-ordered assembly: slots per work item
+constexpr float kDMin = 1e-6f;       // floor of diag(J^T J) in the damping matrix (C5)
+
+// Scalars of the PCG recurrence, device resident (no host round trip inside the loop).
+struct PcgScalars {
+  double rz[2];   // r.z, parity = iteration & 1
+  double pDp[2];  // p.(lambda D_c p), parity = iteration & 1
+  double pq;      // sum_i u_i.e_i of the current matvec
+  double rr;      // |r|^2 after the current update
+  double bnorm2;  // |b|^2
+  double rz0;
+  int done;       // set once converged / broken down: every later kernel returns immediately
+  int converged;
+  int breakdown;  // p.Sp <= 0 or non-finite
+  int iters;
+};
+
+// Scalars of one LM step.
+struct StepScalars {
+  double cost;        // sum_i rho(|r_i|^2)   (F = cost / 2)
+  double trial_cost;  // same at the trial point
+  double jd2;         // |J delta|^2
+  double dg;          // delta.g
+  int bad_block;      // a 9x9 / 3x3 block was not positive definite
+  int pad;
+};
+
+// Everything the kernels need, passed by value.
+struct View {
+  int nc, np, np_obs;  // cameras, points, points with at least one observation (internal ids [0, np_obs))
+  int T, num_tiles;
+  long long n_slots;
+  int num_chunks;
+  int robust;
+  float robust_c2;
+  int damping_mode;
+  // caller's arrays (borrowed)
+  float* cameras;
+  float* points;
+  // per slot
+  const float2* px;
+  const int* cam;
+  const unsigned short* rank;
+  const int* obs_of_slot;  // caller observation id of a slot (-1 = padding)
+  float4* J[6];
+  float2* res;
+  // per tile
+  const int* tile_pt;     // [num_tiles + 1] first internal point of each tile
+  const int* run_begin;   // [num_tiles + 1] index of the tile's first run in run_cam / run_slot
+  const int* run_cam;     // camera id of each run; one terminator (-1) per tile
+  const unsigned short* run_slot;  // first slot (within the tile) of each run; terminator = valid slots
+  // per internal point
+  const int* pt_ptr;      // [np_obs + 1] prefix sum of track lengths
+  const int* pt_perm;     // [np] internal -> caller point id
+  float4* pts;            // current points, internal order (w unused)
+  float4* pts_trial;
+  float4* V0;             // V_k: xx xy xz yy
+  float2* V1;             // V_k: yz zz
+  float4* gp;             // g_p,k (xyz, w unused)
+  float4* Vinv0;          // V'^-1: xx xy xz yy
+  float2* Vinv1;          // V'^-1: yz zz
+  float4* dp;             // delta_p,k
+  // per camera
+  float* cams_trial;      // [nc][9]
+  float* cam_table;       // [nc][28]
+  float* cam_table_trial;
+  double* Ug;             // [nc][54]
+  double* Minv;           // [nc][81]
+  double* lamD;           // [9 nc]
+  double* b;              // [9 nc] Schur right-hand side
+  double* x;              // [9 nc] delta_c
+  double* r;              // [9 nc]
+  double* z;              // [9 nc]
+  double* p;              // [9 nc]
+  double* q;              // [9 nc] matvec accumulator (without the lambda D_c p term)
+  float* p32;             // [nc][12]
+  // camera-ordered assembly work list
+  const int* chunk_cam;   // [num_chunks]
+  const int* chunk_begin; // [num_chunks + 1] into cslot
+  const int* cslot;       // slots grouped by camera, ascending
+  PcgScalars* pcg;
+  StepScalars* step;
+};
+
+// Host-side result of the S0 reordering (ba_reorder.cpp).
+struct Reordered {
+  int T = 0, num_tiles = 0, np_obs = 0;
+  long long n_slots = 0;
+  std::vector<int> obs_of_slot;           // [n_slots]
+  std::vector<int> cam;                   // [n_slots]
+  std::vector<unsigned short> rank;       // [n_slots]
+  std::vector<int> tile_pt;               // [num_tiles + 1]
+  std::vector<int> run_begin;             // [num_tiles + 1]
+  std::vector<int> run_cam;
+  std::vector<unsigned short> run_slot;
+  std::vector<int> pt_ptr;                // [np_obs + 1]
+  std::vector<int> pt_perm;               // [np]
+  std::vector<int> chunk_cam, chunk_begin, cslot;
+  long long camera_runs = 0;
+};
+
+// Returns 0, or CASPAR_BA_EINVAL with `err` set.
+int reorder_observations(int nc, int np, long long n, const int* cam_idx, const int* pt_idx, int forced_tile,
+                         Reordered* out, std::string* err);
+
+// ---- kernel launchers (ba_kernels.cu); all enqueue on `s` and return the launch status ----
+cudaError_t launch_gather_observations(const View& v, const float* observations, float2* px_out, cudaStream_t s);
+cudaError_t launch_pack_points(const View& v, const float* points_caller, float4* dst, cudaStream_t s);
+cudaError_t launch_unpack_points(const View& v, const float4* src, float* points_caller, cudaStream_t s);
+cudaError_t launch_camera_prepass(const View& v, const float* cams, float* table, cudaStream_t s);
+cudaError_t launch_linearize(const View& v, cudaStream_t s);
+cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_acc, cudaStream_t s);
+cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s);
+cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s);
+cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);
+cudaError_t launch_pcg_init(const View& v, cudaStream_t s);
+cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s);
+cudaError_t launch_pcg_update(const View& v, int iter, double tol2, cudaStream_t s);  // two kernels
+cudaError_t launch_backsub(const View& v, cudaStream_t s);
+cudaError_t launch_trial_update(const View& v, cudaStream_t s);
+cudaError_t launch_commit(const View& v, cudaStream_t s);
+cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s);
+cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s);
+int kernels_per(const char* op);  // how many kernels each launcher enqueues (for the launch counter)
+
+}  // namespace cba

@@ -1,0 +1,962 @@
+// ba_kernels.cu — hand-written sm_100a kernels of the bundle-adjustment hot path (steps S1-S9).
+//
+// Everything here is HBM-bandwidth bound scan / gather / segmented-reduce work (about 1 flop per byte
+// in the Schur matvec), so there is no tensor-core path: the design rules are coalesced 128-bit
+// accesses on slot-major arrays, one observation per thread with its Jacobian in registers,
+// shared-memory staging for the two segmented reductions, and one fp64 RED per (tile, camera run)
+// instead of a global atomic per observation.
+//
+// Block-level pattern shared by linearize / Schur pass (one TILE of whole points per block):
+//   * POINT side  — values are scattered to `stage[c][rank]` (rank = position in the tile's
+//     point-major order, so a point's observations are contiguous there); one thread per point sums
+//     its range and writes the per-point result back into the same range for the observations to read.
+//   * CAMERA side — slots are already sorted by camera inside the tile, so `stage[c][slot]` holds
+//     contiguous camera runs; one thread per (run, component) sums the run in fp32 and issues ONE
+//     fp64 atomic add to the L2-resident per-camera accumulator (cross-tile accumulation in fp64).
+#include <math_constants.h>
+
+#include "ba_internal.h"
+
+namespace cba {
+
+static thread_local long long g_launches = 0;
+long long take_launch_count() {
+  long long n = g_launches;
+  g_launches = 0;
+  return n;
+}
+#define CBA_LAUNCHED() (++g_launches, cudaGetLastError())
+
+// ------------------------------------------------------------------------------------------------
+// reductions
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Sum over the block; the result is valid in thread 0.  `red` holds >= 32 doubles.
+__device__ __forceinline__ double block_sum(double v, double* red) {
+  v = warp_sum(v);
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  __syncthreads();
+  if (lane == 0) red[w] = v;
+  __syncthreads();
+  if (w == 0) {
+    v = (lane < (int)(blockDim.x >> 5)) ? red[lane] : 0.0;
+    v = warp_sum(v);
+  }
+  return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S0 helpers: gather the caller's observations into slot order; pack / unpack points
+// ------------------------------------------------------------------------------------------------
+__global__ void gather_observations_kernel(View v, const float* __restrict__ observations, float2* __restrict__ px) {
+  long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= v.n_slots) return;
+  int o = v.obs_of_slot[s];
+  px[s] = o >= 0 ? reinterpret_cast<const float2*>(observations)[o] : make_float2(0.f, 0.f);
+}
+
+__global__ void pack_points_kernel(View v, const float* __restrict__ src, float4* __restrict__ dst) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= v.np) return;
+  const float* p = src + 3ll * v.pt_perm[k];
+  dst[k] = make_float4(p[0], p[1], p[2], 0.f);
+}
+
+__global__ void unpack_points_kernel(View v, const float4* __restrict__ src, float* __restrict__ dst) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= v.np) return;
+  float4 p = src[k];
+  float* d = dst + 3ll * v.pt_perm[k];
+  d[0] = p.x; d[1] = p.y; d[2] = p.z;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S1 camera prepass: everything that depends on the camera alone, once per camera, in fp64.
+// Table row (28 floats): R[9] | C_hi[3] | C_lo[3] | w[3] | f k1 k2 | a b a1 b1 th2 | pad[2]
+// with C = -R^T t the camera centre split into two floats, so that P = R (X - C) is evaluated
+// without the cancellation of R X + t for scenes far from the origin.
+// ------------------------------------------------------------------------------------------------
+__global__ void camera_prepass_kernel(int nc, const float* __restrict__ cams, float* __restrict__ table) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nc) return;
+  const float* c = cams + 9ll * j;
+  const double w0 = c[0], w1 = c[1], w2 = c[2], t0 = c[3], t1 = c[4], t2 = c[5];
+  const double th2 = w0 * w0 + w1 * w1 + w2 * w2;
+  double a, b, a1, b1;
+  if (th2 < 1e-3) {  // Taylor series in th2 (5 terms: truncation below 1e-17 here)
+    a = 1.0 + th2 * (-1.0 / 6 + th2 * (1.0 / 120 + th2 * (-1.0 / 5040 + th2 * (1.0 / 362880))));
+    b = 0.5 + th2 * (-1.0 / 24 + th2 * (1.0 / 720 + th2 * (-1.0 / 40320 + th2 * (1.0 / 3628800))));
+    a1 = -1.0 / 3 + th2 * (1.0 / 30 + th2 * (-1.0 / 840 + th2 * (1.0 / 45360 + th2 * (-1.0 / 3991680))));
+    b1 = -1.0 / 12 + th2 * (1.0 / 180 + th2 * (-1.0 / 6720 + th2 * (1.0 / 453600 + th2 * (-1.0 / 47900160))));
+  } else {
+    const double th = sqrt(th2);
+    double sn, cs;
+    sincos(th, &sn, &cs);
+    const double omc = 2.0 * sin(0.5 * th) * sin(0.5 * th);  // 1 - cos(th) without cancellation
+    a = sn / th;
+    b = omc / th2;
+    a1 = (th * cs - sn) / (th2 * th);
+    b1 = (th * sn - 2.0 * omc) / (th2 * th2);
+  }
+  // R = I + a [w]x + b (w w^T - th2 I)
+  double R[9];
+  R[0] = 1.0 + b * (w0 * w0 - th2); R[1] = -a * w2 + b * w0 * w1;     R[2] = a * w1 + b * w0 * w2;
+  R[3] = a * w2 + b * w1 * w0;      R[4] = 1.0 + b * (w1 * w1 - th2); R[5] = -a * w0 + b * w1 * w2;
+  R[6] = -a * w1 + b * w2 * w0;     R[7] = a * w0 + b * w2 * w1;      R[8] = 1.0 + b * (w2 * w2 - th2);
+  const double C0 = -(R[0] * t0 + R[3] * t1 + R[6] * t2);
+  const double C1 = -(R[1] * t0 + R[4] * t1 + R[7] * t2);
+  const double C2 = -(R[2] * t0 + R[5] * t1 + R[8] * t2);
+  float* o = table + (long long)kCamTableFloats * j;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) o[i] = (float)R[i];
+  const float h0 = (float)C0, h1 = (float)C1, h2 = (float)C2;
+  o[9] = h0; o[10] = h1; o[11] = h2;
+  o[12] = (float)(C0 - (double)h0); o[13] = (float)(C1 - (double)h1); o[14] = (float)(C2 - (double)h2);
+  o[15] = c[0]; o[16] = c[1]; o[17] = c[2];
+  o[18] = c[6]; o[19] = c[7]; o[20] = c[8];
+  o[21] = (float)a; o[22] = (float)b; o[23] = (float)a1; o[24] = (float)b1; o[25] = (float)th2;
+  o[26] = 0.f; o[27] = 0.f;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2 per-observation arithmetic (registers only).  PAPER.md:194-203; O1/O2.
+// ------------------------------------------------------------------------------------------------
+struct Projection {
+  float px, py, n, rad, inz, r0, r1;  // p, |p|^2, radial factor, -1/P_z, residual
+};
+
+__device__ __forceinline__ Projection project(const float4 t0, const float4 t1, const float4 t2, const float4 t3,
+                                              float f, float k1, float k2, float X0, float X1, float X2, float2 m) {
+  // d = X - C (two-float centre), P = R d
+  const float d0 = (X0 - t2.y) - t3.x, d1 = (X1 - t2.z) - t3.y, d2 = (X2 - t2.w) - t3.z;
+  const float P0 = fmaf(t0.x, d0, fmaf(t0.y, d1, t0.z * d2));
+  const float P1 = fmaf(t0.w, d0, fmaf(t1.x, d1, t1.y * d2));
+  const float P2 = fmaf(t1.z, d0, fmaf(t1.w, d1, t2.x * d2));
+  Projection o;
+  o.inz = -__frcp_rn(P2);  // one shared reciprocal
+  o.px = P0 * o.inz;
+  o.py = P1 * o.inz;
+  o.n = fmaf(o.px, o.px, o.py * o.py);
+  o.rad = fmaf(o.n, fmaf(k2, o.n, k1), 1.0f);
+  const float fr = f * o.rad;
+  o.r0 = fmaf(fr, o.px, -m.x);
+  o.r1 = fmaf(fr, o.py, -m.y);
+  return o;
+}
+
+// Full linearization of one observation: J[0..17] = d r / d camera (2x9 row-major), J[18..23] = d r / d point.
+__device__ __forceinline__ void linearize_observation(const float* __restrict__ table, int cam, float X0, float X1,
+                                                      float X2, float2 m, float (&J)[24], float& r0, float& r1) {
+  const float4* row = reinterpret_cast<const float4*>(table) + 7ll * cam;
+  const float4 t0 = __ldg(row + 0), t1 = __ldg(row + 1), t2 = __ldg(row + 2), t3 = __ldg(row + 3);
+  const float4 t4 = __ldg(row + 4), t5 = __ldg(row + 5), t6 = __ldg(row + 6);
+  const float w0 = t3.w, w1 = t4.x, w2 = t4.y, f = t4.z, k1 = t4.w, k2 = t5.x;
+  const float a = t5.y, b = t5.z, a1 = t5.w, b1 = t6.x, th2 = t6.y;
+  const Projection pr = project(t0, t1, t2, t3, f, k1, k2, X0, X1, X2, m);
+  r0 = pr.r0;
+  r1 = pr.r1;
+  const float px = pr.px, py = pr.py, n = pr.n, rad = pr.rad, inz = pr.inz;
+  // d uv / d p = f (rad I + c p p^T), c = 2 k1 + 4 k2 n;  d p / d P = inz [[1, 0, px], [0, 1, py]]
+  const float fc = f * fmaf(4.0f * k2, n, 2.0f * k1);
+  const float fr = f * rad;
+  const float D00 = fmaf(fc * px, px, fr), D01 = fc * px * py, D11 = fmaf(fc * py, py, fr);
+  const float A00 = inz * D00, A01 = inz * D01, A02 = inz * fmaf(D00, px, D01 * py);
+  const float A10 = A01, A11 = inz * D11, A12 = inz * fmaf(D01, px, D11 * py);
+  // d(R X)/d w = u w^T + b w X^T + b s I - a [X]x,  u = a1 q + b1 (w s - th2 X) - 2 b X,  q = w x X, s = w.X
+  const float q0 = w1 * X2 - w2 * X1, q1 = w2 * X0 - w0 * X2, q2 = w0 * X1 - w1 * X0;
+  const float s = fmaf(w0, X0, fmaf(w1, X1, w2 * X2));
+  const float bs = b * s;
+  const float u0 = fmaf(a1, q0, fmaf(b1, fmaf(w0, s, -th2 * X0), -2.0f * b * X0));
+  const float u1 = fmaf(a1, q1, fmaf(b1, fmaf(w1, s, -th2 * X1), -2.0f * b * X1));
+  const float u2 = fmaf(a1, q2, fmaf(b1, fmaf(w2, s, -th2 * X2), -2.0f * b * X2));
+  const float bw0 = b * w0, bw1 = b * w1, bw2 = b * w2;
+  const float aX0 = a * X0, aX1 = a * X1, aX2 = a * X2;
+  // G[i][j] = u_i w_j + bw_i X_j + bs delta_ij - a [X]x_ij   with [X]x = [[0,-X2,X1],[X2,0,-X0],[-X1,X0,0]]
+  const float G00 = fmaf(u0, w0, fmaf(bw0, X0, bs)), G01 = fmaf(u0, w1, fmaf(bw0, X1, aX2)), G02 = fmaf(u0, w2, fmaf(bw0, X2, -aX1));
+  const float G10 = fmaf(u1, w0, fmaf(bw1, X0, -aX2)), G11 = fmaf(u1, w1, fmaf(bw1, X1, bs)), G12 = fmaf(u1, w2, fmaf(bw1, X2, aX0));
+  const float G20 = fmaf(u2, w0, fmaf(bw2, X0, aX1)), G21 = fmaf(u2, w1, fmaf(bw2, X1, -aX0)), G22 = fmaf(u2, w2, fmaf(bw2, X2, bs));
+  J[0] = fmaf(A00, G00, fmaf(A01, G10, A02 * G20));
+  J[1] = fmaf(A00, G01, fmaf(A01, G11, A02 * G21));
+  J[2] = fmaf(A00, G02, fmaf(A01, G12, A02 * G22));
+  J[3] = A00; J[4] = A01; J[5] = A02;
+  J[6] = rad * px;
+  const float fn = f * n;
+  J[7] = fn * px;
+  J[8] = fn * n * px;
+  J[9] = fmaf(A10, G00, fmaf(A11, G10, A12 * G20));
+  J[10] = fmaf(A10, G01, fmaf(A11, G11, A12 * G21));
+  J[11] = fmaf(A10, G02, fmaf(A11, G12, A12 * G22));
+  J[12] = A10; J[13] = A11; J[14] = A12;
+  J[15] = rad * py;
+  J[16] = fn * py;
+  J[17] = fn * n * py;
+  // J_p = A R
+  J[18] = fmaf(A00, t0.x, fmaf(A01, t0.w, A02 * t1.z));
+  J[19] = fmaf(A00, t0.y, fmaf(A01, t1.x, A02 * t1.w));
+  J[20] = fmaf(A00, t0.z, fmaf(A01, t1.y, A02 * t2.x));
+  J[21] = fmaf(A10, t0.x, fmaf(A11, t0.w, A12 * t1.z));
+  J[22] = fmaf(A10, t0.y, fmaf(A11, t1.x, A12 * t1.w));
+  J[23] = fmaf(A10, t0.z, fmaf(A11, t1.y, A12 * t2.x));
+}
+
+__device__ __forceinline__ void residual_observation(const float* __restrict__ table, int cam, float X0, float X1,
+                                                     float X2, float2 m, float& r0, float& r1) {
+  const float4* row = reinterpret_cast<const float4*>(table) + 7ll * cam;
+  const float4 t0 = __ldg(row + 0), t1 = __ldg(row + 1), t2 = __ldg(row + 2), t3 = __ldg(row + 3);
+  const float4 t4 = __ldg(row + 4), t5 = __ldg(row + 5);
+  const Projection pr = project(t0, t1, t2, t3, t4.z, t4.w, t5.x, X0, X1, X2, m);
+  r0 = pr.r0;
+  r1 = pr.r1;
+}
+
+constexpr int blocks_per_sm(int T) { return T == 256 ? 3 : (T == 512 ? 2 : 1); }
+
+// ------------------------------------------------------------------------------------------------
+// S2 + S3 (JAC = true): linearize every observation, store r and J, assemble V_k and g_p,k per point,
+//                       accumulate the cost.
+// S9      (JAC = false): residual-only cost at the given points / camera table.
+// ------------------------------------------------------------------------------------------------
+template <int T, bool JAC>
+__global__ void __launch_bounds__(T, blocks_per_sm(T))
+linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict__ table, double* cost_acc) {
+  __shared__ float stage[JAC ? 9 : 3][T + 1];
+  __shared__ double red[32];
+  const int t = blockIdx.x, tid = threadIdx.x;
+  const long long slot = (long long)t * T + tid;
+  const int p0 = v.tile_pt[t], p1 = v.tile_pt[t + 1];
+  const int base = v.pt_ptr[p0];
+  const int cam = v.cam[slot];
+  const unsigned rank = v.rank[slot];
+  const float2 m = v.px[slot];
+
+  // point threads: scatter X_k to the point's range of ranks
+  for (int k = p0 + tid; k < p1; k += T) {
+    const float4 X = pts[k];
+    const int e = v.pt_ptr[k + 1] - base;
+    for (int r = v.pt_ptr[k] - base; r < e; ++r) {
+      stage[0][r] = X.x; stage[1][r] = X.y; stage[2][r] = X.z;
+    }
+  }
+  __syncthreads();
+
+  float term = 0.f;
+  if (JAC) {
+    float J[24], r0 = 0.f, r1 = 0.f;
+#pragma unroll
+    for (int i = 0; i < 24; ++i) J[i] = 0.f;
+    if (cam >= 0) {
+      linearize_observation(table, cam, stage[0][rank], stage[1][rank], stage[2][rank], m, J, r0, r1);
+      const float s2 = fmaf(r0, r0, r1 * r1);
+      if (v.robust) {  // Cauchy: w = 1 / (1 + s/c^2), r~ = sqrt(w) r, J~ = sqrt(w) J
+        const float q = s2 / v.robust_c2;
+        const float sw = sqrtf(1.0f / (1.0f + q));
+        term = v.robust_c2 * log1pf(q);
+        r0 *= sw; r1 *= sw;
+#pragma unroll
+        for (int i = 0; i < 24; ++i) J[i] *= sw;
+      } else {
+        term = s2;
+      }
+    }
+    // eager stores: six 128-bit chunk arrays + the residual
+#pragma unroll
+    for (int c = 0; c < 6; ++c) v.J[c][slot] = make_float4(J[4 * c], J[4 * c + 1], J[4 * c + 2], J[4 * c + 3]);
+    v.res[slot] = make_float2(r0, r1);
+    __syncthreads();  // every thread has read its X
+    if (cam >= 0) {
+      stage[0][rank] = fmaf(J[18], J[18], J[21] * J[21]);
+      stage[1][rank] = fmaf(J[18], J[19], J[21] * J[22]);
+      stage[2][rank] = fmaf(J[18], J[20], J[21] * J[23]);
+      stage[3][rank] = fmaf(J[19], J[19], J[22] * J[22]);
+      stage[4][rank] = fmaf(J[19], J[20], J[22] * J[23]);
+      stage[5][rank] = fmaf(J[20], J[20], J[23] * J[23]);
+      stage[6][rank] = fmaf(J[18], r0, J[21] * r1);
+      stage[7][rank] = fmaf(J[19], r0, J[22] * r1);
+      stage[8][rank] = fmaf(J[20], r0, J[23] * r1);
+    }
+    __syncthreads();
+    for (int k = p0 + tid; k < p1; k += T) {
+      float acc[9];
+#pragma unroll
+      for (int c = 0; c < 9; ++c) acc[c] = 0.f;
+      const int e = v.pt_ptr[k + 1] - base;
+      for (int r = v.pt_ptr[k] - base; r < e; ++r) {
+#pragma unroll
+        for (int c = 0; c < 9; ++c) acc[c] += stage[c][r];
+      }
+      v.V0[k] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+      v.V1[k] = make_float2(acc[4], acc[5]);
+      v.gp[k] = make_float4(acc[6], acc[7], acc[8], 0.f);
+    }
+  } else {
+    if (cam >= 0) {
+      float r0, r1;
+      residual_observation(table, cam, stage[0][rank], stage[1][rank], stage[2][rank], m, r0, r1);
+      const float s2 = fmaf(r0, r0, r1 * r1);
+      term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
+    }
+  }
+  const double total = block_sum((double)term, red);
+  if (tid == 0) atomicAdd(cost_acc, total);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S4 camera-side assembly: U_j = sum J_c^T J_c (45 unique) and g_c,j = sum J_c^T r (9).
+// Camera-ordered pass: one warp per chunk of <= kChunkSlots slots of one camera (slots ascending, so
+// the gathers walk the camera's in-tile runs contiguously); 54 fp32 partial sums per lane, reduced
+// across lanes in fp64, then one fp64 add per entry.  No per-observation atomics, no hot-camera storm.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) assemble_cameras_kernel(View v) {
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (w >= v.num_chunks) return;
+  const int cam = v.chunk_cam[w];
+  const int b = v.chunk_begin[w], e = v.chunk_begin[w + 1];
+  float acc[kUg];
+#pragma unroll
+  for (int i = 0; i < kUg; ++i) acc[i] = 0.f;
+  for (int i = b + lane; i < e; i += 32) {
+    const int s = v.cslot[i];
+    float J[20];
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+      const float4 x = v.J[c][s];
+      J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
+    }
+    const float2 r = v.res[s];
+    int k = 0;
+#pragma unroll
+    for (int a = 0; a < 9; ++a)
+#pragma unroll
+      for (int c = a; c < 9; ++c) {
+        acc[k] = fmaf(J[a], J[c], fmaf(J[9 + a], J[9 + c], acc[k]));
+        ++k;
+      }
+#pragma unroll
+    for (int a = 0; a < 9; ++a) acc[45 + a] = fmaf(J[a], r.x, fmaf(J[9 + a], r.y, acc[45 + a]));
+  }
+  double mine0 = 0.0, mine1 = 0.0;
+#pragma unroll
+  for (int i = 0; i < kUg; ++i) {
+    const double tot = warp_sum((double)acc[i]);
+    if ((i & 31) == lane) {
+      if (i < 32) mine0 = tot; else mine1 = tot;
+    }
+  }
+  double* dst = v.Ug + (long long)kUg * cam;
+  atomicAdd(dst + lane, mine0);
+  if (lane + 32 < kUg) atomicAdd(dst + lane + 32, mine1);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Damped blocks for one lambda: M^-1 = (U + lambda D_c)^-1 per camera (fp64 Cholesky), lambda D_c,
+// the initial Schur right-hand side -g_c; V'^-1 = (V + lambda D_p)^-1 per point (fp64, stored fp32).
+// ------------------------------------------------------------------------------------------------
+__global__ void prepare_cameras_kernel(View v, double lambda) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= v.nc) return;
+  const double* ug = v.Ug + (long long)kUg * j;
+  double A[81], L[81];
+  {
+    int k = 0;
+    for (int a = 0; a < 9; ++a)
+      for (int c = a; c < 9; ++c) {
+        A[9 * a + c] = ug[k];
+        A[9 * c + a] = ug[k];
+        ++k;
+      }
+  }
+  for (int a = 0; a < 9; ++a) {
+    const double d = v.damping_mode == 1 ? 1.0 : fmax(A[10 * a], (double)kDMin);
+    v.lamD[9ll * j + a] = lambda * d;
+    A[10 * a] += lambda * d;
+    v.b[9ll * j + a] = -ug[45 + a];
+  }
+  bool ok = true;
+  for (int i = 0; i < 81; ++i) L[i] = 0.0;
+  for (int i = 0; i < 9 && ok; ++i)
+    for (int c = 0; c <= i; ++c) {
+      double s = A[9 * i + c];
+      for (int k = 0; k < c; ++k) s -= L[9 * i + k] * L[9 * c + k];
+      if (i == c) {
+        if (!(s > 0.0)) { ok = false; break; }
+        L[10 * i] = sqrt(s);
+      } else {
+        L[9 * i + c] = s / L[10 * c];
+      }
+    }
+  double* Mi = v.Minv + 81ll * j;
+  if (!ok) {
+    v.step->bad_block = 1;
+    for (int i = 0; i < 81; ++i) Mi[i] = (i % 10 == 0) ? 1.0 : 0.0;
+    return;
+  }
+  for (int c = 0; c < 9; ++c) {  // solve L L^T x = e_c
+    double y[9], x[9];
+    for (int i = 0; i < 9; ++i) {
+      double s = (i == c) ? 1.0 : 0.0;
+      for (int k = 0; k < i; ++k) s -= L[9 * i + k] * y[k];
+      y[i] = s / L[10 * i];
+    }
+    for (int i = 8; i >= 0; --i) {
+      double s = y[i];
+      for (int k = i + 1; k < 9; ++k) s -= L[9 * k + i] * x[k];
+      x[i] = s / L[10 * i];
+    }
+    for (int i = 0; i < 9; ++i) Mi[9 * i + c] = x[i];
+  }
+}
+
+__global__ void prepare_points_kernel(View v, double lambda) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= v.np_obs) return;
+  const float4 a = v.V0[k];
+  const float2 c = v.V1[k];
+  double xx = a.x, xy = a.y, xz = a.z, yy = a.w, yz = c.x, zz = c.y;
+  const bool unit = v.damping_mode == 1;
+  xx += lambda * (unit ? 1.0 : fmax(xx, (double)kDMin));
+  yy += lambda * (unit ? 1.0 : fmax(yy, (double)kDMin));
+  zz += lambda * (unit ? 1.0 : fmax(zz, (double)kDMin));
+  // Cholesky pivots decide positive definiteness; the inverse itself is the adjugate over the determinant
+  const double l00 = xx, l10 = xy / l00, l20 = xz / l00;
+  const double d1 = yy - l10 * xy, m21 = yz - l10 * xz, d2 = zz - l20 * xz - (m21 / d1) * m21;
+  if (!(l00 > 0.0) || !(d1 > 0.0) || !(d2 > 0.0)) {
+    v.step->bad_block = 1;
+    v.Vinv0[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    v.Vinv1[k] = make_float2(0.f, 0.f);
+    return;
+  }
+  const double c00 = yy * zz - yz * yz, c01 = xz * yz - xy * zz, c02 = xy * yz - xz * yy;
+  const double c11 = xx * zz - xz * xz, c12 = xy * xz - xx * yz, c22 = xx * yy - xy * xy;
+  const double idet = 1.0 / (xx * c00 + xy * c01 + xz * c02);
+  v.Vinv0[k] = make_float4((float)(c00 * idet), (float)(c01 * idet), (float)(c02 * idet), (float)(c11 * idet));
+  v.Vinv1[k] = make_float2((float)(c12 * idet), (float)(c22 * idet));
+}
+
+// ------------------------------------------------------------------------------------------------
+// S5 / S6 / S8: one pass over the stored Jacobians in tile order.
+//   MATVEC : q_j += sum_{i in j} J_c^T (u - J_p s_k),  u = J_c p_j,  s_k = V'^-1 sum_{i in k} J_p^T u
+//            (the lambda D_c p term and the dot p.q are completed by the PCG update kernel)
+//   RHS    : b_j += sum_{i in j} J_c^T J_p V'^-1 g_p,k          (b_j was initialised to -g_c,j)
+//   BACKSUB: delta_p,k = -V'^-1 (g_p,k + sum_{i in k} J_p^T J_c delta_c,j);  also |J delta|^2, delta_p.g_p
+// ------------------------------------------------------------------------------------------------
+enum { MATVEC = 0, RHS = 1, BACKSUB = 2 };
+
+template <int T, int MODE>
+__global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v, int iter) {
+  __shared__ float stage[9][T + 1];
+  __shared__ double red[32];
+  const int t = blockIdx.x, tid = threadIdx.x;
+  if (MODE == MATVEC) {
+    if (v.pcg->done) return;
+    if (t == 0 && tid == 0) {  // accumulators of the update that follows this matvec
+      const int nxt = (iter + 1) & 1;
+      v.pcg->rz[nxt] = 0.0;
+      v.pcg->pDp[nxt] = 0.0;
+      v.pcg->rr = 0.0;
+    }
+  }
+  const long long slot = (long long)t * T + tid;
+  const int p0 = v.tile_pt[t], p1 = v.tile_pt[t + 1];
+  const int base = v.pt_ptr[p0];
+  const int cam = v.cam[slot];
+  const unsigned rank = v.rank[slot];
+  float J[24];
+#pragma unroll
+  for (int c = 0; c < 6; ++c) {
+    const float4 x = __ldcs(&v.J[c][slot]);  // streamed once per pass: evict-first
+    J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
+  }
+  float u0 = 0.f, u1 = 0.f;
+  if (MODE != RHS) {
+    if (cam >= 0) {
+      const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
+      const float4 a = __ldg(pv), b = __ldg(pv + 1), c = __ldg(pv + 2);
+      const float pj[9] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x};
+#pragma unroll
+      for (int i = 0; i < 9; ++i) {
+        u0 = fmaf(J[i], pj[i], u0);
+        u1 = fmaf(J[9 + i], pj[i], u1);
+      }
+      stage[0][rank] = fmaf(J[18], u0, J[21] * u1);
+      stage[1][rank] = fmaf(J[19], u0, J[22] * u1);
+      stage[2][rank] = fmaf(J[20], u0, J[23] * u1);
+    }
+    __syncthreads();
+  }
+  // point threads
+  float dg_part = 0.f;
+  for (int k = p0 + tid; k < p1; k += T) {
+    const int rb = v.pt_ptr[k] - base, re = v.pt_ptr[k + 1] - base;
+    float t0 = 0.f, t1 = 0.f, t2 = 0.f;
+    if (MODE != RHS)
+      for (int r = rb; r < re; ++r) { t0 += stage[0][r]; t1 += stage[1][r]; t2 += stage[2][r]; }
+    const float4 vi = v.Vinv0[k];
+    const float2 vj = v.Vinv1[k];
+    float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (MODE != MATVEC) {
+      g = v.gp[k];
+      t0 += g.x; t1 += g.y; t2 += g.z;
+    }
+    float s0 = fmaf(vi.x, t0, fmaf(vi.y, t1, vi.z * t2));
+    float s1 = fmaf(vi.y, t0, fmaf(vi.w, t1, vj.x * t2));
+    float s2 = fmaf(vi.z, t0, fmaf(vj.x, t1, vj.y * t2));
+    if (MODE == BACKSUB) {
+      s0 = -s0; s1 = -s1; s2 = -s2;
+      v.dp[k] = make_float4(s0, s1, s2, 0.f);
+      dg_part += fmaf(s0, g.x, fmaf(s1, g.y, s2 * g.z));
+    }
+    for (int r = rb; r < re; ++r) { stage[0][r] = s0; stage[1][r] = s1; stage[2][r] = s2; }
+  }
+  __syncthreads();
+  float c9[9];
+  float dot_part = 0.f;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) c9[i] = 0.f;
+  if (cam >= 0) {
+    const float s0 = stage[0][rank], s1 = stage[1][rank], s2 = stage[2][rank];
+    const float w0 = fmaf(J[18], s0, fmaf(J[19], s1, J[20] * s2));
+    const float w1 = fmaf(J[21], s0, fmaf(J[22], s1, J[23] * s2));
+    if (MODE == BACKSUB) {
+      const float y0 = u0 + w0, y1 = u1 + w1;  // (J delta)_i
+      dot_part = fmaf(y0, y0, y1 * y1);
+    } else {
+      const float e0 = (MODE == MATVEC) ? u0 - w0 : w0;
+      const float e1 = (MODE == MATVEC) ? u1 - w1 : w1;
+      if (MODE == MATVEC) dot_part = fmaf(u0, e0, u1 * e1);
+#pragma unroll
+      for (int i = 0; i < 9; ++i) c9[i] = fmaf(J[i], e0, J[9 + i] * e1);
+    }
+  }
+  if (MODE != BACKSUB) {
+    __syncthreads();  // every thread has read its s_k
+#pragma unroll
+    for (int i = 0; i < 9; ++i) stage[i][tid] = c9[i];
+    __syncthreads();
+    // camera runs: one thread per (run, component), fp32 inside the tile, fp64 across tiles
+    const int rb = v.run_begin[t], nruns = v.run_begin[t + 1] - rb - 1;
+    double* dst = (MODE == MATVEC) ? v.q : v.b;
+    for (int w = tid; w < 9 * nruns; w += T) {
+      const int u = w / 9, a = w - 9 * u;
+      const int s1 = v.run_slot[rb + u + 1];
+      float acc = 0.f;
+      for (int s = v.run_slot[rb + u]; s < s1; ++s) acc += stage[a][s];
+      atomicAdd(dst + 9ll * v.run_cam[rb + u] + a, (double)acc);
+    }
+  }
+  if (MODE == MATVEC) {
+    const double tot = block_sum((double)dot_part, red);
+    if (tid == 0) atomicAdd(&v.pcg->pq, tot);
+  }
+  if (MODE == BACKSUB) {
+    const double jd2 = block_sum((double)dot_part, red);
+    const double dg = block_sum((double)dg_part, red);
+    if (tid == 0) {
+      atomicAdd(&v.step->jd2, jd2);
+      atomicAdd(&v.step->dg, dg);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S7 PCG vector kernels: fp64 state, 32 cameras (288 elements) per block, scalars stay on the device.
+// ------------------------------------------------------------------------------------------------
+constexpr int kPcgThreads = 288;
+
+__device__ __forceinline__ double apply_minv(const View& v, int j, int a, const double* rs_cam) {
+  const double* Mi = v.Minv + 81ll * j + 9 * a;
+  double z = 0.0;
+#pragma unroll
+  for (int c = 0; c < 9; ++c) z = fma(Mi[c], rs_cam[c], z);
+  return z;
+}
+
+// x = 0, r = b, z = M^-1 r, p = z; rz[0], |b|^2, pDp[0]
+__global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v) {
+  __shared__ double rs[kPcgThreads];
+  __shared__ double red[32];
+  const int tid = threadIdx.x;
+  const long long i = (long long)blockIdx.x * kPcgThreads + tid;
+  const int j = (int)(i / 9), a = (int)(i - 9ll * j);
+  const bool valid = j < v.nc;
+  const double ri = valid ? v.b[i] : 0.0;
+  rs[tid] = ri;
+  __syncthreads();
+  double zi = 0.0, ld = 0.0;
+  if (valid) {
+    zi = apply_minv(v, j, a, rs + (tid - a));
+    ld = v.lamD[i];
+    v.x[i] = 0.0;
+    v.r[i] = ri;
+    v.z[i] = zi;
+    v.p[i] = zi;
+    v.q[i] = 0.0;
+    v.p32[(long long)kCamPad * j + a] = (float)zi;
+  }
+  const double s_rz = block_sum(ri * zi, red);
+  const double s_rr = block_sum(ri * ri, red);
+  const double s_pd = block_sum(ld * zi * zi, red);
+  if (tid == 0) {
+    atomicAdd(&v.pcg->rz[0], s_rz);
+    atomicAdd(&v.pcg->bnorm2, s_rr);
+    atomicAdd(&v.pcg->rr, s_rr);
+    atomicAdd(&v.pcg->pDp[0], s_pd);
+  }
+}
+
+// alpha = rz / (p.q); x += alpha p; r -= alpha q; z = M^-1 r; rz_new, |r|^2
+__global__ void __launch_bounds__(kPcgThreads) pcg_update_xr_kernel(View v, int iter) {
+  __shared__ double rs[kPcgThreads];
+  __shared__ double red[32];
+  PcgScalars* sc = v.pcg;
+  if (sc->done) return;
+  const int tid = threadIdx.x, par = iter & 1;
+  const double denom = sc->pq + sc->pDp[par];
+  const double rz = sc->rz[par];
+  if (!(denom > 0.0) || !isfinite(denom) || !isfinite(rz)) {  // breakdown (C15) or b = 0
+    if (blockIdx.x == 0 && tid == 0) {
+      sc->done = 1;
+      if (sc->bnorm2 == 0.0) sc->converged = 1; else sc->breakdown = 1;
+    }
+    return;
+  }
+  const double alpha = rz / denom;
+  const long long i = (long long)blockIdx.x * kPcgThreads + tid;
+  const int j = (int)(i / 9), a = (int)(i - 9ll * j);
+  const bool valid = j < v.nc;
+  double ri = 0.0;
+  if (valid) {
+    const double pi = v.p[i];
+    const double qi = v.q[i] + v.lamD[i] * pi;
+    v.x[i] += alpha * pi;
+    ri = v.r[i] - alpha * qi;
+    v.r[i] = ri;
+  }
+  rs[tid] = ri;
+  __syncthreads();
+  double zi = 0.0;
+  if (valid) {
+    zi = apply_minv(v, j, a, rs + (tid - a));
+    v.z[i] = zi;
+  }
+  const double s_rz = block_sum(ri * zi, red);
+  const double s_rr = block_sum(ri * ri, red);
+  if (tid == 0) {
+    atomicAdd(&sc->rz[par ^ 1], s_rz);
+    atomicAdd(&sc->rr, s_rr);
+    if (blockIdx.x == 0) {
+      sc->iters = iter + 1;
+      if (iter == 0) sc->rz0 = rz;
+    }
+  }
+}
+
+// stop if |r| <= tol |b|, else beta = rz_new / rz; p = z + beta p; p.(lambda D p); q = 0
+__global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v, int iter, double tol2) {
+  __shared__ double red[32];
+  PcgScalars* sc = v.pcg;
+  if (sc->done) return;
+  const int tid = threadIdx.x, par = iter & 1;
+  if (sc->rr <= tol2 * sc->bnorm2) {
+    if (blockIdx.x == 0 && tid == 0) { sc->done = 1; sc->converged = 1; }
+    return;
+  }
+  const double beta = sc->rz[par ^ 1] / sc->rz[par];
+  const long long i = (long long)blockIdx.x * kPcgThreads + tid;
+  const int j = (int)(i / 9), a = (int)(i - 9ll * j);
+  double pd = 0.0;
+  if (j < v.nc) {
+    const double pi = v.z[i] + beta * v.p[i];
+    v.p[i] = pi;
+    v.q[i] = 0.0;
+    v.p32[(long long)kCamPad * j + a] = (float)pi;
+    pd = v.lamD[i] * pi * pi;
+  }
+  const double s_pd = block_sum(pd, red);
+  if (tid == 0) {
+    atomicAdd(&sc->pDp[par ^ 1], s_pd);
+    if (blockIdx.x == 0) sc->pq = 0.0;
+  }
+}
+
+// delta_c -> fp32 padded copy for the back-substitution pass; delta_c . g_c
+__global__ void __launch_bounds__(kPcgThreads) delta_c_kernel(View v) {
+  __shared__ double red[32];
+  const long long i = (long long)blockIdx.x * kPcgThreads + threadIdx.x;
+  const int j = (int)(i / 9), a = (int)(i - 9ll * j);
+  double d = 0.0;
+  if (j < v.nc) {
+    const double xi = v.x[i];
+    v.p32[(long long)kCamPad * j + a] = (float)xi;
+    d = xi * v.Ug[(long long)kUg * j + 45 + a];
+  }
+  const double s = block_sum(d, red);
+  if (threadIdx.x == 0) atomicAdd(&v.step->dg, s);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S9 trial point and commit
+// ------------------------------------------------------------------------------------------------
+__global__ void trial_update_kernel(View v) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < 9ll * v.nc) v.cams_trial[i] = (float)((double)v.cameras[i] + v.x[i]);
+  if (i < v.np) {
+    const float4 p = v.pts[i], d = v.dp[i];
+    v.pts_trial[i] = make_float4(p.x + d.x, p.y + d.y, p.z + d.z, 0.f);
+  }
+}
+
+__global__ void commit_kernel(View v) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < 9ll * v.nc) v.cameras[i] = v.cams_trial[i];
+  if (i < v.np) {
+    const float4 p = v.pts_trial[i];
+    v.pts[i] = p;
+    float* d = v.points + 3ll * v.pt_perm[i];
+    d[0] = p.x; d[1] = p.y; d[2] = p.z;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// test-only exports (caller order, fp64 array-of-structs) and the standalone matvec
+// ------------------------------------------------------------------------------------------------
+__global__ void export_kernel(View v, int what, double* __restrict__ dst) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  switch (what) {
+    case CASPAR_BA_RESIDUALS:
+    case CASPAR_BA_JC:
+    case CASPAR_BA_JP: {
+      if (i >= v.n_slots) return;
+      const int o = v.obs_of_slot[i];
+      if (o < 0) return;
+      if (what == CASPAR_BA_RESIDUALS) {
+        const float2 r = v.res[i];
+        dst[2ll * o] = r.x;
+        dst[2ll * o + 1] = r.y;
+      } else {
+        float J[24];
+        for (int c = 0; c < 6; ++c) {
+          const float4 x = v.J[c][i];
+          J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
+        }
+        if (what == CASPAR_BA_JC)
+          for (int e = 0; e < 18; ++e) dst[18ll * o + e] = J[e];
+        else
+          for (int e = 0; e < 6; ++e) dst[6ll * o + e] = J[18 + e];
+      }
+      return;
+    }
+    case CASPAR_BA_U: {
+      if (i >= v.nc) return;
+      const double* ug = v.Ug + (long long)kUg * i;
+      int k = 0;
+      for (int a = 0; a < 9; ++a)
+        for (int c = a; c < 9; ++c) {
+          dst[81ll * i + 9 * a + c] = ug[k];
+          dst[81ll * i + 9 * c + a] = ug[k];
+          ++k;
+        }
+      return;
+    }
+    case CASPAR_BA_V: {
+      if (i >= v.np) return;
+      double* d = dst + 9ll * v.pt_perm[i];
+      if (i >= v.np_obs) {
+        for (int e = 0; e < 9; ++e) d[e] = 0.0;
+        return;
+      }
+      const float4 a = v.V0[i];
+      const float2 c = v.V1[i];
+      d[0] = a.x; d[1] = a.y; d[2] = a.z; d[3] = a.y; d[4] = a.w; d[5] = c.x; d[6] = a.z; d[7] = c.x; d[8] = c.y;
+      return;
+    }
+    case CASPAR_BA_G:
+    case CASPAR_BA_DELTA: {
+      const bool grad = what == CASPAR_BA_G;
+      if (i < 9ll * v.nc) {
+        const int j = (int)(i / 9), a = (int)(i - 9ll * j);
+        dst[i] = grad ? v.Ug[(long long)kUg * j + 45 + a] : v.x[i];
+      }
+      if (i < v.np) {
+        double* d = dst + 9ll * v.nc + 3ll * v.pt_perm[i];
+        const float4 g = grad ? v.gp[i] : v.dp[i];
+        const bool live = i < v.np_obs;
+        d[0] = live ? g.x : 0.0; d[1] = live ? g.y : 0.0; d[2] = live ? g.z : 0.0;
+      }
+      return;
+    }
+    case CASPAR_BA_SCHUR_RHS:
+      if (i < 9ll * v.nc) dst[i] = v.b[i];
+      return;
+  }
+}
+
+__global__ void matvec_load_kernel(View v, const double* __restrict__ p_in) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 9ll * v.nc) return;
+  const int j = (int)(i / 9), a = (int)(i - 9ll * j);
+  v.p[i] = p_in[i];
+  v.q[i] = 0.0;
+  v.p32[(long long)kCamPad * j + a] = (float)p_in[i];
+}
+
+__global__ void matvec_finish_kernel(View v, double* __restrict__ q_out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 9ll * v.nc) return;
+  q_out[i] = v.q[i] + v.lamD[i] * v.p[i];
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+static inline unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
+
+cudaError_t launch_gather_observations(const View& v, const float* observations, float2* px_out, cudaStream_t s) {
+  if (v.n_slots == 0) return cudaSuccess;
+  gather_observations_kernel<<<grid_for(v.n_slots, 256), 256, 0, s>>>(v, observations, px_out);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_pack_points(const View& v, const float* src, float4* dst, cudaStream_t s) {
+  if (v.np == 0) return cudaSuccess;
+  pack_points_kernel<<<grid_for(v.np, 256), 256, 0, s>>>(v, src, dst);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_unpack_points(const View& v, const float4* src, float* dst, cudaStream_t s) {
+  if (v.np == 0) return cudaSuccess;
+  unpack_points_kernel<<<grid_for(v.np, 256), 256, 0, s>>>(v, src, dst);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_camera_prepass(const View& v, const float* cams, float* table, cudaStream_t s) {
+  if (v.nc == 0) return cudaSuccess;
+  camera_prepass_kernel<<<grid_for(v.nc, 128), 128, 0, s>>>(v.nc, cams, table);
+  return CBA_LAUNCHED();
+}
+
+template <bool JAC>
+static cudaError_t launch_linearize_t(const View& v, const float4* pts, const float* table, double* acc,
+                                      cudaStream_t s) {
+  if (v.num_tiles == 0) return cudaSuccess;
+  switch (v.T) {
+    case 256: linearize_kernel<256, JAC><<<v.num_tiles, 256, 0, s>>>(v, pts, table, acc); break;
+    case 512: linearize_kernel<512, JAC><<<v.num_tiles, 512, 0, s>>>(v, pts, table, acc); break;
+    default: linearize_kernel<1024, JAC><<<v.num_tiles, 1024, 0, s>>>(v, pts, table, acc); break;
+  }
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_linearize(const View& v, cudaStream_t s) {
+  return launch_linearize_t<true>(v, v.pts, v.cam_table, &v.step->cost, s);
+}
+
+cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_acc, cudaStream_t s) {
+  return launch_linearize_t<false>(v, pts, table, cost_acc, s);
+}
+
+cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s) {
+  if (v.num_chunks == 0) return cudaSuccess;
+  assemble_cameras_kernel<<<grid_for(32ll * v.num_chunks, 128), 128, 0, s>>>(v);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s) {
+  cudaError_t e = cudaSuccess;
+  if (v.nc > 0) {
+    prepare_cameras_kernel<<<grid_for(v.nc, 64), 64, 0, s>>>(v, lambda);
+    e = CBA_LAUNCHED();
+  }
+  if (e == cudaSuccess && v.np_obs > 0) {
+    prepare_points_kernel<<<grid_for(v.np_obs, 256), 256, 0, s>>>(v, lambda);
+    e = CBA_LAUNCHED();
+  }
+  return e;
+}
+
+template <int MODE>
+static cudaError_t launch_pass(const View& v, int iter, cudaStream_t s) {
+  if (v.num_tiles == 0) return cudaSuccess;
+  switch (v.T) {
+    case 256: schur_pass_kernel<256, MODE><<<v.num_tiles, 256, 0, s>>>(v, iter); break;
+    case 512: schur_pass_kernel<512, MODE><<<v.num_tiles, 512, 0, s>>>(v, iter); break;
+    default: schur_pass_kernel<1024, MODE><<<v.num_tiles, 1024, 0, s>>>(v, iter); break;
+  }
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pass<RHS>(v, 0, s); }
+cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) { return launch_pass<MATVEC>(v, iter, s); }
+
+cudaError_t launch_pcg_init(const View& v, cudaStream_t s) {
+  if (v.nc == 0) return cudaSuccess;
+  pcg_init_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_pcg_update(const View& v, int iter, double tol2, cudaStream_t s) {
+  if (v.nc == 0) return cudaSuccess;
+  const unsigned g = grid_for(9ll * v.nc, kPcgThreads);
+  pcg_update_xr_kernel<<<g, kPcgThreads, 0, s>>>(v, iter);
+  cudaError_t e = CBA_LAUNCHED();
+  if (e != cudaSuccess) return e;
+  pcg_update_p_kernel<<<g, kPcgThreads, 0, s>>>(v, iter, tol2);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_backsub(const View& v, cudaStream_t s) {
+  cudaError_t e = cudaSuccess;
+  if (v.nc > 0) {
+    delta_c_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
+    e = CBA_LAUNCHED();
+  }
+  if (e != cudaSuccess) return e;
+  return launch_pass<BACKSUB>(v, 0, s);
+}
+
+cudaError_t launch_trial_update(const View& v, cudaStream_t s) {
+  const long long n = 9ll * v.nc > v.np ? 9ll * v.nc : v.np;
+  if (n == 0) return cudaSuccess;
+  trial_update_kernel<<<grid_for(n, 256), 256, 0, s>>>(v);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_commit(const View& v, cudaStream_t s) {
+  const long long n = 9ll * v.nc > v.np ? 9ll * v.nc : v.np;
+  if (n == 0) return cudaSuccess;
+  commit_kernel<<<grid_for(n, 256), 256, 0, s>>>(v);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s) {
+  long long n = 0;
+  switch (what) {
+    case CASPAR_BA_RESIDUALS: case CASPAR_BA_JC: case CASPAR_BA_JP: n = v.n_slots; break;
+    case CASPAR_BA_U: n = v.nc; break;
+    case CASPAR_BA_V: n = v.np; break;
+    case CASPAR_BA_G: case CASPAR_BA_DELTA: n = 9ll * v.nc > v.np ? 9ll * v.nc : v.np; break;
+    case CASPAR_BA_SCHUR_RHS: n = 9ll * v.nc; break;
+    default: return cudaErrorInvalidValue;
+  }
+  if (n == 0) return cudaSuccess;
+  export_kernel<<<grid_for(n, 256), 256, 0, s>>>(v, what, dst);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s) {
+  if (v.nc == 0) return cudaSuccess;
+  const unsigned g = grid_for(9ll * v.nc, 256);
+  matvec_load_kernel<<<g, 256, 0, s>>>(v, p_in);
+  cudaError_t e = CBA_LAUNCHED();
+  if (e != cudaSuccess) return e;
+  e = launch_pass<MATVEC>(v, 0, s);
+  if (e != cudaSuccess) return e;
+  matvec_finish_kernel<<<g, 256, 0, s>>>(v, q_out);
+  return CBA_LAUNCHED();
+}
+
+}  // namespace cba

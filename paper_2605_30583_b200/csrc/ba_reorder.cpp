@@ -1,0 +1,182 @@
+// ba_reorder.cpp — step S0: one-off reordering of the observations at create (host side).
+//
+// "observations reordered (sorted by point, with camera-side segments)" — BASELINE.json north_star.
+// The tile metadata built here plays the role of the paper's SharedIndex arrays:
+// a block-local sorted list of unique camera indices plus a per-thread target, built once and reused
+// by every kernel.  Nothing below is copied from the paper; it describes no algorithm for this.
+//
+//   1. points are ordered by (lowest camera id that observes them, caller id): points that share
+//      cameras end up in the same tile, which keeps the number of camera runs per tile small;
+//      unobserved points go last and belong to no tile;
+//   2. points are packed greedily into tiles of at most T observations (whole points only);
+//   3. inside a tile, slots are sorted by (camera id, internal point id): equal-camera runs are
+//      contiguous; `rank` gives each slot's position in the tile's point-major order;
+//   4. a camera-ordered list of slots (chunks of <= kChunkSlots) drives the camera-block assembly.
+#include <algorithm>
+#include <cstdlib>
+#include <numeric>
+
+#include "ba_internal.h"
+
+namespace cba {
+
+int reorder_observations(int nc, int np, long long n, const int* cam_idx, const int* pt_idx, int forced_tile,
+                         Reordered* out, std::string* err) {
+  if (n >= (1LL << 31) - 4096) {
+    *err = "more than 2^31 observations are not supported";
+    return CASPAR_BA_EINVAL;
+  }
+  // --- validate, count tracks, lowest camera per point -----------------------------------------
+  std::vector<int> track(np, 0), key(np, nc);
+  for (long long i = 0; i < n; ++i) {
+    int c = cam_idx[i], k = pt_idx[i];
+    if (c < 0 || c >= nc || k < 0 || k >= np) {
+      *err = "camera_index / point_index out of range at observation " + std::to_string(i);
+      return CASPAR_BA_EINVAL;
+    }
+    track[k]++;
+    if (c < key[k]) key[k] = c;
+  }
+  int max_track = 0;
+  for (int k = 0; k < np; ++k) max_track = std::max(max_track, track[k]);
+  if (max_track > CASPAR_BA_MAX_TRACK) {
+    *err = "a point has " + std::to_string(max_track) + " observations; the limit is " +
+           std::to_string(CASPAR_BA_MAX_TRACK);
+    return CASPAR_BA_EINVAL;
+  }
+  int T = forced_tile;
+  if (T == 0) T = (max_track <= 256 && n <= (1LL << 20)) ? 256 : 512;
+  while (T < max_track) T *= 2;
+  if (T != 256 && T != 512 && T != 1024) {
+    *err = "tile size must be 256, 512 or 1024";
+    return CASPAR_BA_EINVAL;
+  }
+
+  // --- 1. internal point order: counting sort by key (stable -> ties by caller id) --------------
+  std::vector<int> bucket(nc + 2, 0);
+  for (int k = 0; k < np; ++k) bucket[key[k] + 1]++;
+  for (int c = 0; c <= nc; ++c) bucket[c + 1] += bucket[c];
+  std::vector<int>& perm = out->pt_perm;
+  perm.assign(np, 0);
+  std::vector<int> internal_of(np);
+  {
+    std::vector<int> fill(bucket.begin(), bucket.end() - 1);
+    for (int k = 0; k < np; ++k) {
+      int pos = fill[key[k]]++;
+      perm[pos] = k;
+      internal_of[k] = pos;
+    }
+  }
+  int np_obs = bucket[nc];  // points with key < nc, i.e. observed at least once
+  out->np_obs = np_obs;
+  out->pt_ptr.assign(np_obs + 1, 0);
+  for (int a = 0; a < np_obs; ++a) out->pt_ptr[a + 1] = out->pt_ptr[a] + track[perm[a]];
+
+  // observations grouped by internal point (caller's order inside a point)
+  std::vector<int> obs_by_pt(n > 0 ? n : 1);
+  {
+    std::vector<int> fill(out->pt_ptr.begin(), out->pt_ptr.end() - 1);
+    for (long long i = 0; i < n; ++i) obs_by_pt[fill[internal_of[pt_idx[i]]]++] = (int)i;
+  }
+
+  // --- 2. greedy tiles of whole points ---------------------------------------------------------
+  std::vector<int>& tile_pt = out->tile_pt;
+  tile_pt.clear();
+  tile_pt.push_back(0);
+  {
+    int used = 0;
+    for (int a = 0; a < np_obs; ++a) {
+      int len = track[perm[a]];
+      if (used + len > T) {
+        tile_pt.push_back(a);
+        used = 0;
+      }
+      used += len;
+    }
+    if (np_obs > 0) tile_pt.push_back(np_obs);
+  }
+  int num_tiles = (int)tile_pt.size() - 1;
+  out->T = T;
+  out->num_tiles = num_tiles;
+  out->n_slots = (long long)num_tiles * T;
+  out->obs_of_slot.assign(out->n_slots > 0 ? out->n_slots : 1, -1);
+  out->cam.assign(out->n_slots > 0 ? out->n_slots : 1, -1);
+  out->rank.assign(out->n_slots > 0 ? out->n_slots : 1, 0);
+  out->run_begin.assign(num_tiles + 1, 0);
+
+  // --- 3. in-tile sort by (camera, point-major position) and run tables -------------------------
+  std::vector<int> runs_per_tile(num_tiles, 0);
+#pragma omp parallel
+  {
+    std::vector<unsigned long long> keys;
+#pragma omp for schedule(dynamic, 64)
+    for (int t = 0; t < num_tiles; ++t) {
+      int base = out->pt_ptr[tile_pt[t]];
+      int cnt = out->pt_ptr[tile_pt[t + 1]] - base;
+      keys.resize(cnt);
+      for (int r = 0; r < cnt; ++r)  // r = position in point-major order
+        keys[r] = ((unsigned long long)cam_idx[obs_by_pt[base + r]] << 16) | (unsigned)r;
+      std::sort(keys.begin(), keys.end());
+      long long s0 = (long long)t * T;
+      int runs = 0, prev = -1;
+      for (int s = 0; s < cnt; ++s) {
+        int r = (int)(keys[s] & 0xFFFFu), c = (int)(keys[s] >> 16);
+        out->obs_of_slot[s0 + s] = obs_by_pt[base + r];
+        out->cam[s0 + s] = c;
+        out->rank[s0 + s] = (unsigned short)r;
+        if (c != prev) { runs++; prev = c; }
+      }
+      runs_per_tile[t] = runs;
+    }
+  }
+  long long total_runs = 0;
+  for (int t = 0; t < num_tiles; ++t) {
+    out->run_begin[t] = (int)(total_runs + t);  // + t: one terminator entry per earlier tile
+    total_runs += runs_per_tile[t];
+  }
+  out->run_begin[num_tiles] = (int)(total_runs + num_tiles);
+  out->camera_runs = total_runs;
+  out->run_cam.assign(total_runs + num_tiles + 1, -1);
+  out->run_slot.assign(total_runs + num_tiles + 1, 0);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int t = 0; t < num_tiles; ++t) {
+    long long s0 = (long long)t * T;
+    int cnt = out->pt_ptr[tile_pt[t + 1]] - out->pt_ptr[tile_pt[t]];
+    int w = out->run_begin[t], prev = -1;
+    for (int s = 0; s < cnt; ++s) {
+      int c = out->cam[s0 + s];
+      if (c != prev) {
+        out->run_cam[w] = c;
+        out->run_slot[w] = (unsigned short)s;
+        ++w;
+        prev = c;
+      }
+    }
+    out->run_cam[w] = -1;  // terminator: first slot past the tile's valid ones
+    out->run_slot[w] = (unsigned short)cnt;
+  }
+
+  // --- 4. camera-ordered slot list in chunks ---------------------------------------------------
+  std::vector<long long> cptr(nc + 1, 0);
+  for (long long i = 0; i < n; ++i) cptr[cam_idx[i] + 1]++;
+  for (int c = 0; c < nc; ++c) cptr[c + 1] += cptr[c];
+  out->cslot.assign(n > 0 ? n : 1, 0);
+  {
+    std::vector<long long> fill(cptr.begin(), cptr.end() - 1);
+    for (long long s = 0; s < out->n_slots; ++s) {  // ascending slots -> each camera's list is ascending
+      int c = out->cam[s];
+      if (c >= 0) out->cslot[fill[c]++] = (int)s;
+    }
+  }
+  out->chunk_cam.clear();
+  out->chunk_begin.clear();
+  for (int c = 0; c < nc; ++c)
+    for (long long b = cptr[c]; b < cptr[c + 1]; b += kChunkSlots) {
+      out->chunk_cam.push_back(c);
+      out->chunk_begin.push_back((int)b);
+    }
+  out->chunk_begin.push_back((int)n);
+  return 0;
+}
+
+}  // namespace cba
