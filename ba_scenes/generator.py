@@ -59,6 +59,7 @@ CONFIGS: Dict[str, dict] = {
 GRID_SPACING = 2.0
 GRID_HEIGHT = 10.0
 RING_RADIUS = 10.0
+MAX_DEPTH = -5.0            # every generated observation has P_z <= MAX_DEPTH at the true parameters
 
 
 @dataclasses.dataclass
@@ -243,10 +244,12 @@ def _visibility_zipf(rng, n_cameras: int, length: np.ndarray, s: float):
 # forward projection (measurement synthesis only)
 # ---------------------------------------------------------------------------
 def _project(cameras: np.ndarray, points: np.ndarray, cam_idx: np.ndarray, pt_idx: np.ndarray,
-             chunk: int = 1 << 21) -> np.ndarray:
-    """uv = f r p with p = -P_xy / P_z, r = 1 + k1 |p|^2 + k2 |p|^4 (configs[0])."""
+             chunk: int = 1 << 21) -> Tuple[np.ndarray, np.ndarray]:
+    """uv = f r p with p = -P_xy / P_z, r = 1 + k1 |p|^2 + k2 |p|^4 (configs[0]).
+    Returns (uv [N, 2], depth P_z [N])."""
     rot = Rotation.from_rotvec(cameras[:, 0:3]).as_matrix()
     out = np.empty((cam_idx.shape[0], 2), dtype=np.float64)
+    depth = np.empty(cam_idx.shape[0], dtype=np.float64)
     for s in range(0, cam_idx.shape[0], chunk):
         c = cam_idx[s:s + chunk]
         k = pt_idx[s:s + chunk]
@@ -255,7 +258,8 @@ def _project(cameras: np.ndarray, points: np.ndarray, cam_idx: np.ndarray, pt_id
         n2 = np.sum(p * p, axis=1)
         r = 1.0 + cameras[c, 7] * n2 + cameras[c, 8] * n2 * n2
         out[s:s + chunk] = (cameras[c, 6] * r)[:, None] * p
-    return out
+        depth[s:s + chunk] = pc[:, 2]
+    return out, depth
 
 
 # ---------------------------------------------------------------------------
@@ -315,7 +319,15 @@ def make_scene(name: str, *, noise_free: bool = False, seed: Optional[int] = Non
     n_obs = pt_idx.shape[0]
 
     # --- measurements -------------------------------------------------------------------
-    uv = _project(cams_true.astype(np.float64), pts_true.astype(np.float64), cam_idx, pt_idx)
+    uv, depth = _project(cams_true.astype(np.float64), pts_true.astype(np.float64), cam_idx, pt_idx)
+    # visibility cull (reading C7: no depth guard in the model, so scenes keep P_z <= -5): drop the few
+    # grazing observations, never taking a point below two observations
+    graze = depth > MAX_DEPTH
+    if graze.any():
+        left = np.bincount(pt_idx, minlength=n_pts) - np.bincount(pt_idx[graze], minlength=n_pts)
+        keep = ~(graze & (left[pt_idx] >= 2))
+        uv, cam_idx, pt_idx = uv[keep], cam_idx[keep], pt_idx[keep]
+        n_obs = pt_idx.shape[0]
     noise = rng.normal(0.0, 1.0, size=(n_obs, 2))
     outlier = rng.random(n_obs) < cfg["outlier_fraction"]
     outlier_px = rng.uniform(-cfg.get("outlier_range", 300.0), cfg.get("outlier_range", 300.0), size=(n_obs, 2))
@@ -325,8 +337,17 @@ def make_scene(name: str, *, noise_free: bool = False, seed: Optional[int] = Non
     obs = uv.astype(np.float32)
 
     # --- perturbed start ----------------------------------------------------------------
+    # N(0, 0.01) on rotation / translation, applied in the camera's own frame (reading C16):
+    # R0 = Exp(d_w) R about the camera centre, C0 = C + d_c, t0 = -R0 C0.  Adding the noise to (w, t) of
+    # P = R X + t literally would turn far cameras about the WORLD origin and throw their points by
+    # |X| * 0.01 (up to ~8 units on the large grid), putting hundreds of observations behind the camera.
     cams0 = cams_true.astype(np.float64)
-    cams0[:, 0:6] += rng.normal(0.0, 0.01, size=(n_cam, 6))
+    rot_true = Rotation.from_rotvec(cams0[:, 0:3])
+    centre = -rot_true.inv().apply(cams0[:, 3:6])
+    rot0 = Rotation.from_rotvec(rng.normal(0.0, 0.01, size=(n_cam, 3))) * rot_true
+    centre0 = centre + rng.normal(0.0, 0.01, size=(n_cam, 3))
+    cams0[:, 0:3] = rot0.as_rotvec()
+    cams0[:, 3:6] = -rot0.apply(centre0)
     pts0 = pts_true.astype(np.float64) + rng.normal(0.0, 0.05, size=(n_pts, 3))
 
     if shuffle:

@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py — LM iterations/s (and Schur matvecs/s, HBM roofline fraction) of the B200 bundle-adjustment path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload large]
+
+A "step" is ONE Levenberg-Marquardt iteration of the whole hot path (S1-S10: linearize, block assembly,
+Schur PCG with the config's cap / tolerance, back-substitution, trial cost, accept / reject) on the seeded
+synthetic scene of BASELINE.json configs[3] ("large": 13,700 cameras, 4.5 M points, ~28.8 M observations),
+the scene the north_star's roofline target is quoted on.  The timed K steps are the first K iterations of
+the adaptive LM schedule from the perturbed start (lambda0 = 1e-2); the W warm-up steps run first and the
+parameters are then reset.  One JSON line is printed by rank 0.
+
+N > 1 (torchrun): the path is single-GPU (north_star); ranks run independent replicas of the config with
+different seeds and no data-path collective ("scaling": "weak"); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+LAMBDA0 = 1e-2
+FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+# bounded oracle sample: same recipe as the workload, shrunk (see cpu_baseline.sample)
+SAMPLES = {"large": dict(grid=(24, 32), num_points=250_000), "mid": dict(grid=(15, 20), num_points=160_000),
+           "skewed": dict(num_cameras=600, num_points=120_000), "small": {}, "tiny": {}}
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel: str):
+    """dram bytes per launch of `kernel` from the committed ncu --set full summary, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            return json.load(fh).get(kernel)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self) -> dict:
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1]))
+                mx.append(float(r[2]))
+            except Exception:
+                continue
+            for name, cell in zip(names, r[5:9]):
+                if cell.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def nielsen(lam: float, nu: float, step):
+    if step.accepted:
+        c = 2.0 * step.rho - 1.0
+        return lam * max(1.0 / 3.0, 1.0 - c * c * c), 2.0
+    return lam * nu, 2.0 * nu
+
+
+# ---------------------------------------------------------------------------------------------------
+# reference arm: the fp64 oracle, as it stands, on the host cores
+# ---------------------------------------------------------------------------------------------------
+def time_oracle(workload: str, steps: int, warmup: int, full_observations: int):
+    """LM iterations/s of the oracle on a bounded sample of `workload`; returns (value scaled to the full
+    workload, description dict)."""
+    import oracle
+    from ba_scenes import CONFIGS, make_scene
+
+    scene = make_scene(workload, **SAMPLES[workload])
+    cfg = CONFIGS[workload]
+    ref = oracle.OracleBA.from_scene(scene)
+    lam, nu = LAMBDA0, 2.0
+    matvecs = 0
+    elapsed = 0.0
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        st = ref.lm_step(lam, cfg["pcg_rel_tol"], cfg["pcg_max_iter"], 0)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            elapsed += dt
+            matvecs += st.pcg_iterations
+        lam, nu = nielsen(lam, nu, st)
+    n_s = scene.num_observations
+    per_it_sample = steps / elapsed
+    scale = n_s / max(1, full_observations)
+    desc = {"kind": "oracle", "cores": oracle.num_threads(),
+            "sample": (f"{workload} recipe shrunk to {scene.num_cameras} cameras / {scene.num_points} points / "
+                       f"{n_s} observations; {steps} LM iterations (PCG cap {cfg['pcg_max_iter']}, tol "
+                       f"{cfg['pcg_rel_tol']:g}; {matvecs} matvecs) took {elapsed:.2f} s = {per_it_sample:.3f} it/s on the "
+                       f"sample, scaled by observations ({n_s}/{full_observations}) to the full workload"),
+            "sample_lm_iterations_per_s": per_it_sample, "sample_observations": n_s,
+            "sample_matvecs_per_s": matvecs / elapsed}
+    return per_it_sample * scale, desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from ba_scenes import CONFIGS
+    full_obs = {"large": 28_810_903, "mid": 5_035_057, "skewed": 15_213_972, "small": 129_449, "tiny": 5_990}[args.workload]
+    t0 = time.perf_counter()
+    value, desc = time_oracle(args.workload, args.steps, args.warmup, full_obs)
+    wall = time.perf_counter() - t0
+    desc["value"] = value
+    cfg = CONFIGS[args.workload]
+    line = {"impl": "reference", "metric": "lm_iterations_per_s", "value": value, "unit": "LM iterations/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / value,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"configs[3]-style '{args.workload}' (seed {cfg['seed']}), bounded sample, scaled",
+                       "pcg_max_iter": cfg["pcg_max_iter"], "pcg_rel_tol": cfg["pcg_rel_tol"], "lambda0": LAMBDA0},
+            "cpu_baseline": desc, "gpu_launches": 0, "wall_s": wall,
+            "e2e": {"value": value, "unit": "LM iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2605_30583_b200 as pkg
+    from ba_scenes import CONFIGS, make_scene
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = CONFIGS[args.workload]
+    kw = {}
+    if args.shrink:                                   # debugging only; the bench line says so
+        kw = SAMPLES[args.workload]
+    scene = make_scene(args.workload, seed=cfg["seed"] + 1000 * rank, **kw)
+    n_obs = scene.num_observations
+    cams0 = torch.from_numpy(scene.cameras).to(dev)
+    pts0 = torch.from_numpy(scene.points).to(dev)
+    gpu = pkg.CasparBA(cams0.clone(), pts0.clone(), scene.observations, scene.camera_index, scene.point_index,
+                       scene.robust_loss, scene.robust_scale, 0, device=dev)
+    tol, cap = cfg["pcg_rel_tol"], cfg["pcg_max_iter"]
+
+    def reset():
+        gpu.cameras.copy_(cams0)
+        gpu.points.copy_(pts0)
+        gpu.linearize()                               # parameters changed behind the handle: re-linearize
+
+    def run_steps(k, e2e_buffers=None):
+        lam, nu, out = LAMBDA0, 2.0, []
+        for _ in range(k):
+            if e2e_buffers is not None:
+                gpu.set_parameters_host(*e2e_buffers)
+            st = gpu.lm_step(float(np.float32(lam)), tol, cap, 0)
+            if e2e_buffers is not None:
+                gpu.get_parameters_host(*e2e_buffers)
+            lam, nu = nielsen(lam, nu, st)
+            out.append(st)
+        return out
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident: warm-up, reset, K timed steps --------------------------------------------
+    run_steps(args.warmup)
+    reset()
+    gpu.set_profiling(True)                           # CUDA events around every linearize / matvec launch
+    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clocks:
+        start.record()
+        steps = run_steps(args.steps)
+        stop.record()
+        barrier()
+    ms = start.elapsed_time(stop)
+    st = gpu.stats()
+    gpu.set_profiling(False)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    matvecs = sum(s.pcg_iterations for s in steps)
+    lin_count = int(st.linearize_count)
+
+    # ---- end to end: host buffers, H2D + lm_step + D2H every step ------------------------------------
+    cam_h = torch.empty((scene.num_cameras, 9), dtype=torch.float32).pin_memory()
+    pts_h = torch.empty((scene.num_points, 3), dtype=torch.float32).pin_memory()
+    reset()
+    gpu.get_parameters_host(cam_h, pts_h)
+    run_steps(1, (cam_h, pts_h))
+    cam_h.copy_(torch.from_numpy(scene.cameras))
+    pts_h.copy_(torch.from_numpy(scene.points))
+    barrier()
+    t0 = time.perf_counter()
+    run_steps(args.steps, (cam_h, pts_h))
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    param_bytes = 4 * (9 * scene.num_cameras + 3 * scene.num_points)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (Schur matvec) and of linearize -----------------------------
+    peak, peak_src = hbm_peak()
+    observed_points = int(np.unique(scene.point_index).size)
+    # algorithmic bytes:
+    #   matvec   : J_c 72 + J_p 24 + camera id 4 per observation, V'^-1 24 per observed point
+    #   linearize: pixel 8 + camera id 4 + r 8 + J_c 72 + J_p 24 per observation, X 12 + V,g_p 36 per point
+    mv_bytes = 100.0 * n_obs + 24.0 * observed_points
+    lin_bytes = 116.0 * n_obs + 48.0 * observed_points
+    mv_ms = st.matvec_ms_total / max(1, st.matvec_count)
+    lin_ms = st.linearize_ms_total / max(1, st.linearize_count)
+    mv_gbs = mv_bytes / (mv_ms * 1e-3) / 1e9 if mv_ms > 0 else 0.0
+    lin_gbs = lin_bytes / (lin_ms * 1e-3) / 1e9 if lin_ms > 0 else 0.0
+
+    value = world * args.steps / (ms_max * 1e-3)
+    line = {
+        "metric": "lm_iterations_per_s", "value": value, "unit": "LM iterations/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[3] '{args.workload}' (seed {cfg['seed']})" + (" SHRUNK (debug)" if args.shrink else ""),
+                   "cameras": scene.num_cameras, "points": scene.num_points, "observations": n_obs,
+                   "pcg_max_iter": cap, "pcg_rel_tol": tol, "lambda0": LAMBDA0, "tile_slots": int(st.tile_slots),
+                   "l2": "inputs larger than L2 (stored Jacobians %.2f GB per pass)" % (96.0 * n_obs / 1e9),
+                   "replicas": world, "parallelism": "independent replicas, no collective"},
+        "schur_matvecs_per_s": world * matvecs / (ms_max * 1e-3), "matvecs_in_timed_region": matvecs,
+        "linearizations_per_s": n_obs / (lin_ms * 1e-3) if lin_ms > 0 else None,
+        "lm_costs": [s.cost_after for s in steps], "lm_accepted": [bool(s.accepted) for s in steps],
+        "pcg_iterations": [s.pcg_iterations for s in steps],
+        "roofline": {"kernel": "schur_pass_kernel<T,MATVEC>", "bound": "hbm", "achieved": mv_gbs, "peak": peak,
+                     "unit": "GB/s", "frac": mv_gbs / peak, "traffic": ncu_traffic("schur_matvec"),
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": mv_bytes, "avg_launch_ms": mv_ms,
+                     "launches_timed": int(st.matvec_count), "frac_of_nominal_8TBs": mv_gbs / 8000.0},
+        "roofline_linearize": {"kernel": "linearize_kernel<T,true>", "bound": "hbm", "achieved": lin_gbs, "peak": peak,
+                               "unit": "GB/s", "frac": lin_gbs / peak, "traffic": ncu_traffic("linearize"),
+                               "algorithmic_bytes_per_launch": lin_bytes, "avg_launch_ms": lin_ms,
+                               "launches_timed": lin_count},
+        "e2e": {"value": world * args.steps / e2e_s, "unit": "LM iterations/s", "h2d_bytes_per_step": param_bytes,
+                "d2h_bytes_per_step": param_bytes + 88,
+                "what": "pinned host parameters -> caspar_ba_set_parameters_host, caspar_ba_lm_step, "
+                        "caspar_ba_get_parameters_host + step_info, every step; wall clock"},
+        "gpu_launches": int(st.kernels_launched),
+        "clocks": clocks.summary(),
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        v, desc = time_oracle(args.workload, 1, 0, n_obs)
+        desc["value"] = v
+        desc["unit"] = "LM iterations/s"
+        line["cpu_baseline"] = desc
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="large", choices=list(SAMPLES))
+    ap.add_argument("--shrink", action="store_true", help="debug: run the shrunken sample scene on the GPU")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

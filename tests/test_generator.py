@@ -84,18 +84,30 @@ def test_inputs_are_float32_valid_and_reproducible(scene_cache):
     assert np.unique(key).size == key.size
     again = make_scene("tiny")
     assert np.array_equal(again.observations, s.observations) and np.array_equal(again.cameras, s.cameras)
-    # start is a perturbation of the truth: N(0, 0.01) on rotation/translation, N(0, 0.05) on points
-    assert 0.005 < np.std(s.cameras[:, :6] - s.cameras_true[:, :6]) < 0.02
+    # start is a perturbation of the truth: N(0, 0.01) on rotation and camera centre (in the camera's own
+    # frame, reading C16), N(0, 0.05) on points
+    from scipy.spatial.transform import Rotation
+    r0 = Rotation.from_rotvec(s.cameras[:, :3].astype(np.float64))
+    r1 = Rotation.from_rotvec(s.cameras_true[:, :3].astype(np.float64))
+    assert 0.005 < np.std((r0 * r1.inv()).as_rotvec()) < 0.02
+    c0 = -r0.inv().apply(s.cameras[:, 3:6].astype(np.float64))
+    c1 = -r1.inv().apply(s.cameras_true[:, 3:6].astype(np.float64))
+    assert 0.005 < np.std(c0 - c1) < 0.02
     assert 0.04 < np.std(s.points - s.points_true) < 0.06
     assert np.array_equal(s.cameras[:, 6:], s.cameras_true[:, 6:])
 
 
-@pytest.mark.parametrize("name,kw", [("tiny", {}), ("mid", dict(grid=(8, 10), num_points=3000))])
+@pytest.mark.parametrize("name,kw", [("tiny", {}), ("mid", dict(grid=(8, 10), num_points=3000)),
+                                     ("large", dict(grid=(100, 137), num_points=60_000)),
+                                     ("skewed", dict(num_cameras=300, num_points=5000))])
 def test_points_in_front_of_cameras(name, kw):
-    """Reading C7: no epsilon guard, so every generated observation must have P_z well below zero."""
+    """Reading C7: no epsilon guard, so every generated observation must have P_z well below zero, at the
+    true parameters (<= -5) and at the perturbed start (large keeps the full 100 x 137 grid extent here:
+    the far cameras are the ones a careless start perturbation would break)."""
     from scipy.spatial.transform import Rotation
     s = make_scene(name, **kw)
-    rot = Rotation.from_rotvec(s.cameras[:, :3].astype(np.float64)).as_matrix()
-    pc = np.einsum("nij,nj->ni", rot[s.camera_index], s.points[s.point_index].astype(np.float64))
-    pc += s.cameras[s.camera_index, 3:6]
-    assert pc[:, 2].max() < -5.0
+    for cams, pts, bound in ((s.cameras_true, s.points_true, -5.0 + 1e-4), (s.cameras, s.points, -4.0)):
+        rot = Rotation.from_rotvec(cams[:, :3].astype(np.float64)).as_matrix()
+        pc = np.einsum("nij,nj->ni", rot[s.camera_index], pts[s.point_index].astype(np.float64))
+        pc += cams[s.camera_index, 3:6]
+        assert pc[:, 2].max() < bound

@@ -1,0 +1,147 @@
+"""CPU tests of the CUDA library's host logic: the C-ABI shared library loads without a GPU and exports
+every symbol include/caspar_ba.h declares, and step S0 (the tile reordering) satisfies the invariants the
+kernels rely on.  No compute entry point is called here."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2605_30583_b200 as pkg
+from ba_scenes import make_scene
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_loads_and_exports_the_header():
+    lib = pkg.load_library()
+    with open(os.path.join(ROOT, "include", "caspar_ba.h")) as fh:
+        header = fh.read()
+    declared = set(re.findall(r"\b(caspar_ba_[a-z_]+)\s*\(", header))
+    assert declared, "no declarations found in include/caspar_ba.h"
+    for name in sorted(declared):
+        assert hasattr(lib, name), f"libcaspar_ba.so does not export {name}"
+    assert declared == set(pkg.EXPORTED_SYMBOLS)
+    assert os.path.dirname(pkg.library_path()) == os.path.join(ROOT, "paper_2605_30583_b200")   # in-tree
+
+
+def test_no_oracle_on_the_product_path():
+    """The package must not import, link or execute anything under oracle/ (and vice versa)."""
+    for base, forbidden in (("paper_2605_30583_b200", "oracle"), ("oracle", "paper_2605_30583_b200"),
+                            ("oracle", "caspar_ba"), ("ba_scenes", "oracle"), ("ba_scenes", "paper_2605_30583_b200")):
+        for dirpath, _, files in os.walk(os.path.join(ROOT, base)):
+            for f in files:
+                if f.endswith((".py", ".cu", ".cpp", ".h", ".c")):
+                    with open(os.path.join(dirpath, f)) as fh:
+                        text = fh.read()
+                    hits = [ln for ln in text.splitlines()
+                            if re.search(rf"^\s*(from|import|#include).*\b{forbidden}", ln)]
+                    assert not hits, (os.path.join(dirpath, f), hits)
+
+
+def _check_layout(scene, L):
+    n, T = scene.num_observations, L["T"]
+    obs, cam, rank = L["obs_of_slot"], L["cam"], L["rank"]
+    valid = obs >= 0
+    # every observation sits in exactly one slot, with its own camera id
+    assert valid.sum() == n and np.array_equal(np.sort(obs[valid]), np.arange(n))
+    assert np.array_equal(cam[valid], scene.camera_index[obs[valid]])
+    assert (cam[~valid] == -1).all()
+    # points: internal order is a permutation; observed points first, ordered by lowest camera id
+    perm = L["pt_perm"]
+    assert np.array_equal(np.sort(perm), np.arange(scene.num_points))
+    track = np.bincount(scene.point_index, minlength=scene.num_points)
+    np_obs = L["observed_points"]
+    assert (track[perm[:np_obs]] > 0).all() and (track[perm[np_obs:]] == 0).all()
+    assert np.array_equal(np.diff(L["pt_ptr"]), track[perm[:np_obs]])
+    lowest = np.full(scene.num_points, scene.num_cameras)
+    np.minimum.at(lowest, scene.point_index, scene.camera_index)
+    assert (np.diff(lowest[perm[:np_obs]]) >= 0).all()
+    internal_of = np.empty(scene.num_points, np.int64)
+    internal_of[perm] = np.arange(scene.num_points)
+    # tiles hold whole points, at most T observations, and are filled greedily
+    tile_pt, pt_ptr = L["tile_pt"], L["pt_ptr"].astype(np.int64)
+    assert tile_pt[0] == 0 and tile_pt[-1] == np_obs and (np.diff(tile_pt) > 0).all()
+    counts = pt_ptr[tile_pt[1:]] - pt_ptr[tile_pt[:-1]]
+    assert counts.max() <= T and counts.sum() == n
+    nxt = track[perm[tile_pt[1:-1]]]                        # first point of the next tile did not fit
+    assert (counts[:-1] + nxt > T).all()
+    for t in range(L["num_tiles"]):
+        s0 = t * T
+        c = int(counts[t])
+        sl = slice(s0, s0 + c)
+        assert valid[sl].all() and not valid[s0 + c:s0 + T].any()
+        # the tile's observations belong to exactly the tile's points
+        k = internal_of[scene.point_index[obs[sl]]]
+        assert k.min() >= tile_pt[t] and k.max() < tile_pt[t + 1]
+        # camera runs contiguous: camera ids non-decreasing over the slots
+        assert (np.diff(cam[sl]) >= 0).all()
+        # rank: a permutation of [0, c) that puts each point's observations in its pt_ptr range
+        r = rank[sl].astype(np.int64)
+        assert np.array_equal(np.sort(r), np.arange(c))
+        base = pt_ptr[tile_pt[t]]
+        assert ((r >= pt_ptr[k] - base) & (r < pt_ptr[k + 1] - base)).all()
+        # run table: heads at every change of camera, terminator = number of valid slots
+        rb, re_ = L["run_begin"][t], L["run_begin"][t + 1]
+        heads = np.nonzero(np.r_[True, np.diff(cam[sl]) != 0])[0]
+        assert re_ - rb - 1 == heads.size
+        assert np.array_equal(L["run_slot"][rb:re_ - 1], heads) and L["run_slot"][re_ - 1] == c
+        assert np.array_equal(L["run_cam"][rb:re_ - 1], cam[s0 + heads]) and L["run_cam"][re_ - 1] == -1
+    assert L["camera_runs"] == L["run_begin"][-1] - L["num_tiles"]
+    # camera-ordered chunks: each camera's slots ascending, chunks of at most 1024
+    cslot, cb, cc = L["cslot"], L["chunk_begin"], L["chunk_cam"]
+    assert cb[0] == 0 and cb[-1] == n and (np.diff(cb) > 0).all() and (np.diff(cb) <= 1024).all()
+    assert np.array_equal(np.sort(cslot), np.nonzero(valid)[0])
+    for w in range(L["num_chunks"]):
+        s = cslot[cb[w]:cb[w + 1]]
+        assert (cam[s] == cc[w]).all() and (np.diff(s) > 0).all()
+    per_cam = np.bincount(scene.camera_index, minlength=scene.num_cameras)
+    assert L["num_chunks"] == int(np.sum((per_cam + 1023) // 1024))
+
+
+@pytest.mark.parametrize("name,kw,tile", [
+    ("tiny", {}, 0), ("tiny", {}, 512), ("tiny", {}, 1024),
+    ("large", dict(grid=(10, 14), num_points=20_000), 0),
+    ("skewed", dict(num_cameras=300, num_points=20_000), 0),
+])
+def test_layout_invariants(name, kw, tile):
+    scene = make_scene(name, **kw)
+    L = pkg.plan_layout(scene.num_cameras, scene.num_points, scene.camera_index, scene.point_index, tile)
+    if tile:
+        assert L["T"] == tile
+    _check_layout(scene, L)
+
+
+def test_layout_tile_size_follows_longest_track():
+    # one point seen by 600 cameras: T must grow to 1024; 1025 observations of one point are refused
+    for track, want in ((200, 256), (300, 512), (600, 1024)):
+        ci = np.arange(track, dtype=np.int32)
+        L = pkg.plan_layout(track, 1, ci, np.zeros(track, np.int32))
+        assert L["T"] == want and L["num_tiles"] == 1 and L["camera_runs"] == track
+    with pytest.raises(pkg.CasparError) as e:
+        pkg.plan_layout(2000, 1, np.arange(1025, dtype=np.int32), np.zeros(1025, np.int32))
+    assert e.value.code == -1
+
+
+def test_layout_degenerate_inputs():
+    L = pkg.plan_layout(3, 4, np.zeros(0, np.int32), np.zeros(0, np.int32))          # no observations
+    assert L["num_tiles"] == 0 and L["observed_points"] == 0 and L["padded_slots"] == 0
+    L = pkg.plan_layout(0, 0, np.zeros(0, np.int32), np.zeros(0, np.int32))          # nothing at all
+    assert L["num_tiles"] == 0
+    with pytest.raises(pkg.CasparError):                                             # index out of range
+        pkg.plan_layout(2, 2, np.array([0, 2], np.int32), np.array([0, 1], np.int32))
+    with pytest.raises(pkg.CasparError):
+        pkg.plan_layout(2, 2, np.array([0, 1], np.int32), np.array([0, -1], np.int32))
+    # unobserved points go last and belong to no tile
+    L = pkg.plan_layout(2, 5, np.array([1, 0, 1], np.int32), np.array([3, 3, 1], np.int32))
+    assert L["observed_points"] == 2 and sorted(L["pt_perm"][:2]) == [1, 3] and sorted(L["pt_perm"][2:]) == [0, 2, 4]
+    assert list(L["pt_perm"][:2]) == [3, 1]                                          # lowest camera 0 before 1
+
+
+def test_binding_refuses_to_run_without_a_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    s = make_scene("tiny")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        pkg.CasparBA.from_scene(s)
