@@ -89,6 +89,8 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.run_begin = c.take<int>(ro.run_begin.size());
   v.run_cam = c.take<int>(ro.run_cam.size());
   v.run_slot = c.take<unsigned short>(ro.run_slot.size());
+  v.tile_dir = c.take<int4>(ro.tile_dir.size() / 4);
+  v.tile_meta = c.take<unsigned char>(ro.tile_meta.size());
   v.pt_ptr = c.take<int>(ro.pt_ptr.size());
   v.pt_perm = c.take<int>(NP);
   v.cslot = c.take<int>(ro.cslot.size());
@@ -99,8 +101,7 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.V0 = c.take<float4>(NP);
   v.V1 = c.take<float2>(NP);
   v.gp = c.take<float4>(NP);
-  v.Vinv0 = c.take<float4>(NP);
-  v.Vinv1 = c.take<float2>(NP);
+  v.Vinv = c.take<float4>(2 * NP);
   v.dp = c.take<float4>(NP);
   v.cams_trial = c.take<float>(9 * NC);
   v.cam_table = c.take<float>(kCamTableFloats * NC);
@@ -323,6 +324,14 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   v.damping_mode = pb->damping_mode;
   v.cameras = pb->cameras;
   v.points = pb->points;
+  v.max_pts_per_tile = ro.max_pts_per_tile;
+  v.meta_max_bytes = ro.meta_max_bytes;
+  {
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    v.num_sms = sms > 0 ? sms : 148;
+  }
   h->camera_runs = ro.camera_runs;
   h->arena_bytes = carve(h, nullptr, ro);
   cudaError_t e = cudaMalloc(&h->arena, h->arena_bytes);
@@ -336,6 +345,8 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   if (e == cudaSuccess) e = upload(v.run_begin, ro.run_begin, s);
   if (e == cudaSuccess) e = upload(v.run_cam, ro.run_cam, s);
   if (e == cudaSuccess) e = upload(v.run_slot, ro.run_slot, s);
+  if (e == cudaSuccess) e = upload(v.tile_dir, ro.tile_dir, s);
+  if (e == cudaSuccess) e = upload(v.tile_meta, ro.tile_meta, s);
   if (e == cudaSuccess) e = upload(v.pt_ptr, ro.pt_ptr, s);
   if (e == cudaSuccess) e = upload(v.pt_perm, ro.pt_perm, s);
   if (e == cudaSuccess) e = upload(v.cslot, ro.cslot, s);
@@ -356,6 +367,7 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
     }
     if (e == cudaSuccess) e = launch_gather_observations(v, src, const_cast<float2*>(v.px), s);
   }
+  if (e == cudaSuccess) e = configure_kernels(v);
   if (e == cudaSuccess) e = cudaMallocHost(&h->h_pcg, sizeof(PcgScalars));
   if (e == cudaSuccess) e = cudaMallocHost(&h->h_step, sizeof(StepScalars));
   if (e == cudaSuccess) e = cudaMallocHost(&h->h_flags, 2 * sizeof(int));

@@ -79,6 +79,15 @@ struct View {
   const int* run_begin;   // [num_tiles + 1] index of the tile's first run in run_cam / run_slot
   const int* run_cam;     // camera id of each run; one terminator (-1) per tile
   const unsigned short* run_slot;  // first slot (within the tile) of each run; terminator = valid slots
+  // per tile, for the pipelined (TMA bulk) kernels: one 16-byte aligned metadata blob per tile
+  //   int4 header {npts, nruns, nvalid, first internal point}
+  //   uint16 pt_start[npts + 1]   (rank range of each point, padded to 16 B)
+  //   uint16 run_slot[nruns + 1]  (padded to 16 B)
+  //   int32  run_cam[nruns]       (padded to 16 B)
+  const int4* tile_dir;            // [num_tiles] {blob offset in 16-B units, blob bytes, first point, npts}
+  const unsigned char* tile_meta;  // blobs
+  int max_pts_per_tile, meta_max_bytes;
+  int num_sms;
   // per internal point
   const int* pt_ptr;      // [np_obs + 1] prefix sum of track lengths
   const int* pt_perm;     // [np] internal -> caller point id
@@ -87,8 +96,7 @@ struct View {
   float4* V0;             // V_k: xx xy xz yy
   float2* V1;             // V_k: yz zz
   float4* gp;             // g_p,k (xyz, w unused)
-  float4* Vinv0;          // V'^-1: xx xy xz yy
-  float2* Vinv1;          // V'^-1: yz zz
+  float4* Vinv;           // V'^-1, two float4 per point: (xx xy xz yy) (yz zz 0 0) — 32 B, bulk-copy aligned
   float4* dp;             // delta_p,k
   // per camera
   float* cams_trial;      // [nc][9]
@@ -126,6 +134,9 @@ struct Reordered {
   std::vector<int> pt_ptr;                // [np_obs + 1]
   std::vector<int> pt_perm;               // [np]
   std::vector<int> chunk_cam, chunk_begin, cslot;
+  std::vector<int> tile_dir;              // [4 * num_tiles]
+  std::vector<unsigned char> tile_meta;
+  int max_pts_per_tile = 0, meta_max_bytes = 0;
   long long camera_runs = 0;
 };
 
@@ -145,6 +156,8 @@ cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s);
 cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);
 cudaError_t launch_pcg_init(const View& v, cudaStream_t s);
 cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s);
+cudaError_t configure_kernels(const View& v);  // once per handle: dynamic shared memory opt-in
+bool pipelined_matvec_available(const View& v);
 cudaError_t launch_pcg_update(const View& v, int iter, double tol2, cudaStream_t s);  // two kernels
 cudaError_t launch_backsub(const View& v, cudaStream_t s);
 cudaError_t launch_trial_update(const View& v, cudaStream_t s);

@@ -15,6 +15,8 @@
 //     fp64 atomic add to the L2-resident per-camera accumulator (cross-tile accumulation in fp64).
 #include <math_constants.h>
 
+#include <cstdlib>
+
 #include "ba_internal.h"
 
 namespace cba {
@@ -426,15 +428,15 @@ __global__ void prepare_points_kernel(View v, double lambda) {
   const double d1 = yy - l10 * xy, m21 = yz - l10 * xz, d2 = zz - l20 * xz - (m21 / d1) * m21;
   if (!(l00 > 0.0) || !(d1 > 0.0) || !(d2 > 0.0)) {
     v.step->bad_block = 1;
-    v.Vinv0[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-    v.Vinv1[k] = make_float2(0.f, 0.f);
+    v.Vinv[2ll * k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    v.Vinv[2ll * k + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
     return;
   }
   const double c00 = yy * zz - yz * yz, c01 = xz * yz - xy * zz, c02 = xy * yz - xz * yy;
   const double c11 = xx * zz - xz * xz, c12 = xy * xz - xx * yz, c22 = xx * yy - xy * xy;
   const double idet = 1.0 / (xx * c00 + xy * c01 + xz * c02);
-  v.Vinv0[k] = make_float4((float)(c00 * idet), (float)(c01 * idet), (float)(c02 * idet), (float)(c11 * idet));
-  v.Vinv1[k] = make_float2((float)(c12 * idet), (float)(c22 * idet));
+  v.Vinv[2ll * k] = make_float4((float)(c00 * idet), (float)(c01 * idet), (float)(c02 * idet), (float)(c11 * idet));
+  v.Vinv[2ll * k + 1] = make_float4((float)(c12 * idet), (float)(c22 * idet), 0.f, 0.f);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -495,8 +497,8 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v,
     float t0 = 0.f, t1 = 0.f, t2 = 0.f;
     if (MODE != RHS)
       for (int r = rb; r < re; ++r) { t0 += stage[0][r]; t1 += stage[1][r]; t2 += stage[2][r]; }
-    const float4 vi = v.Vinv0[k];
-    const float2 vj = v.Vinv1[k];
+    const float4 vi = v.Vinv[2ll * k];
+    const float4 vj = v.Vinv[2ll * k + 1];
     float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
     if (MODE != MATVEC) {
       g = v.gp[k];
@@ -559,6 +561,231 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v,
       atomicAdd(&v.step->jd2, jd2);
       atomicAdd(&v.step->dg, dg);
     }
+  }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// S6, pipelined: the Schur matvec as a PERSISTENT kernel, one CTA per SM.
+//
+//   producer warp : one elected lane streams whole tiles into a ring of shared-memory stages with TMA
+//                   bulk copies (cp.async.bulk.shared::cluster.global + mbarrier complete_tx): the six
+//                   Jacobian chunk arrays, camera ids, ranks, the tile's metadata blob and its V'^-1
+//                   rows — ten copies, one mbarrier per stage, L2 evict-first on the streamed Jacobians.
+//   consumer warps: T threads, one observation each, run the three reduction phases of a tile from
+//                   shared memory only; the only global traffic left on their critical path is the
+//                   L1/L2-resident p_j gather and the fire-and-forget fp64 REDs.
+// The ring keeps STAGES-1 tiles (~60 KB each) in flight per SM regardless of what the consumers do,
+// which is what the first (one block per tile) version lacked: ncu showed 38 % barrier + 38 %
+// long-scoreboard stalls at 39 % of HBM peak (profiles/r01_matvec_v1.md).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t"
+      "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar,
+                                         unsigned long long policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
+template <int N>
+__device__ __forceinline__ void consumer_bar() {
+  asm volatile("bar.sync 1, %0;" ::"n"(N) : "memory");
+}
+
+struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
+  int j, cam, rank, vinv, meta, stage_bytes;
+  int stages, pstage, cstage, red, bars, total;
+};
+
+__host__ __device__ inline PipeLayout pipe_layout(int T, int max_pts, int meta_max, int smem_limit) {
+  PipeLayout L;
+  auto up = [](int x) { return (x + 127) & ~127; };
+  L.j = 0;
+  L.cam = L.j + 6 * T * 16;
+  L.rank = L.cam + T * 4;
+  L.vinv = up(L.rank + T * 2);
+  L.meta = up(L.vinv + max_pts * 32);
+  L.stage_bytes = up(L.meta + meta_max);
+  const int fixed = up(3 * (T + 1) * 4) + up(9 * (T + 1) * 4) + 256 + 128;
+  int st = (smem_limit - fixed) / L.stage_bytes;
+  L.stages = st > 4 ? 4 : st;
+  L.pstage = L.stages * L.stage_bytes;
+  L.cstage = L.pstage + up(3 * (T + 1) * 4);
+  L.red = L.cstage + up(9 * (T + 1) * 4);
+  L.bars = L.red + 256;
+  L.total = L.bars + 128;
+  return L;
+}
+
+template <int T>
+__global__ void __launch_bounds__(T + 32, 1) schur_matvec_pipelined_kernel(View v, int iter, PipeLayout L) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  if (v.pcg->done) return;
+  const int tid = threadIdx.x;
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L.bars);
+  unsigned long long* empty = full + 4;
+  if (tid == 0) {
+    for (int s = 0; s < L.stages; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, T / 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (blockIdx.x == 0) {  // accumulators of the update that follows this matvec
+      const int nxt = (iter + 1) & 1;
+      v.pcg->rz[nxt] = 0.0;
+      v.pcg->pDp[nxt] = 0.0;
+      v.pcg->rr = 0.0;
+    }
+  }
+  __syncthreads();
+  const int G = gridDim.x;
+
+  if (tid >= T) {
+    // ===== producer warp: one lane issues every copy =====
+    if (tid == T) {
+      unsigned long long pol_stream, pol_keep;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+      asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+      int s = 0;
+      unsigned ph = 0;
+      int t = blockIdx.x;
+      int4 d = t < v.num_tiles ? __ldg(v.tile_dir + t) : make_int4(0, 0, 0, 0);
+      for (; t < v.num_tiles; t += G) {
+        const int tn = t + G;
+        const int4 dn = tn < v.num_tiles ? __ldg(v.tile_dir + tn) : make_int4(0, 0, 0, 0);  // prefetch next entry
+        mbar_wait(empty + s, ph ^ 1);
+        unsigned char* st = smem + (size_t)s * L.stage_bytes;
+        const unsigned vinv_bytes = (unsigned)d.w * 32u;
+        mbar_expect_tx(full + s, (unsigned)(6 * T * 16 + T * 4 + T * 2) + vinv_bytes + (unsigned)d.y);
+        const long long slot0 = (long long)t * T;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) bulk_g2s(st + L.j + c * T * 16, v.J[c] + slot0, T * 16, full + s, pol_stream);
+        bulk_g2s(st + L.cam, v.cam + slot0, T * 4, full + s, pol_stream);
+        bulk_g2s(st + L.rank, v.rank + slot0, T * 2, full + s, pol_stream);
+        bulk_g2s(st + L.vinv, v.Vinv + 2ll * d.z, vinv_bytes, full + s, pol_keep);
+        bulk_g2s(st + L.meta, v.tile_meta + 16ll * d.x, (unsigned)d.y, full + s, pol_stream);
+        d = dn;
+        if (++s == L.stages) { s = 0; ph ^= 1; }
+      }
+    }
+    return;
+  }
+
+  // ===== consumers =====
+  float(*pstage)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.pstage);
+  float(*cstage)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.cstage);
+  double* red = reinterpret_cast<double*>(smem + L.red);
+  float dot_part = 0.f;
+  int s = 0;
+  unsigned ph = 0;
+  for (int t = blockIdx.x; t < v.num_tiles; t += G) {
+    mbar_wait(full + s, ph);
+    const unsigned char* st = smem + (size_t)s * L.stage_bytes;
+    const int4 hdr = *reinterpret_cast<const int4*>(st + L.meta);
+    const int npts = hdr.x, nruns = hdr.y;
+    const unsigned short* pt_start = reinterpret_cast<const unsigned short*>(st + L.meta + 16);
+    const unsigned short* run_slot = pt_start + ((npts + 1 + 7) & ~7);
+    const int* run_cam = reinterpret_cast<const int*>(run_slot + ((nruns + 1 + 7) & ~7));
+    const int cam = reinterpret_cast<const int*>(st + L.cam)[tid];
+    const unsigned rank = reinterpret_cast<const unsigned short*>(st + L.rank)[tid];
+    // phase A: u = J_c p_j, scatter J_p^T u to the point-major staging rows
+    float4 pa = make_float4(0.f, 0.f, 0.f, 0.f), pb = pa, pc = pa;
+    if (cam >= 0) {
+      const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
+      pa = __ldg(pv); pb = __ldg(pv + 1); pc = __ldg(pv + 2);
+    }
+    float J[24];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      const float4 x = reinterpret_cast<const float4*>(st + L.j + c * T * 16)[tid];
+      J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
+    }
+    float u0 = 0.f, u1 = 0.f;
+    if (cam >= 0) {
+      const float pj[9] = {pa.x, pa.y, pa.z, pa.w, pb.x, pb.y, pb.z, pb.w, pc.x};
+#pragma unroll
+      for (int i = 0; i < 9; ++i) {
+        u0 = fmaf(J[i], pj[i], u0);
+        u1 = fmaf(J[9 + i], pj[i], u1);
+      }
+      pstage[0][rank] = fmaf(J[18], u0, J[21] * u1);
+      pstage[1][rank] = fmaf(J[19], u0, J[22] * u1);
+      pstage[2][rank] = fmaf(J[20], u0, J[23] * u1);
+    }
+    consumer_bar<T>();
+    // phase B: one thread per point: t_k = sum over its rank range, s_k = V'^-1 t_k, written back in place
+    if (tid < npts) {
+      const int rb = pt_start[tid], re = pt_start[tid + 1];
+      float t0 = 0.f, t1 = 0.f, t2 = 0.f;
+      for (int r = rb; r < re; ++r) { t0 += pstage[0][r]; t1 += pstage[1][r]; t2 += pstage[2][r]; }
+      const float4 vi = reinterpret_cast<const float4*>(st + L.vinv)[2 * tid];
+      const float4 vj = reinterpret_cast<const float4*>(st + L.vinv)[2 * tid + 1];
+      const float s0 = fmaf(vi.x, t0, fmaf(vi.y, t1, vi.z * t2));
+      const float s1 = fmaf(vi.y, t0, fmaf(vi.w, t1, vj.x * t2));
+      const float s2 = fmaf(vi.z, t0, fmaf(vj.x, t1, vj.y * t2));
+      for (int r = rb; r < re; ++r) { pstage[0][r] = s0; pstage[1][r] = s1; pstage[2][r] = s2; }
+    }
+    consumer_bar<T>();
+    // phase C: e = u - J_p s_k, c = J_c^T e into the slot-major (camera-run) staging rows
+    {
+      float c9[9];
+#pragma unroll
+      for (int i = 0; i < 9; ++i) c9[i] = 0.f;
+      if (cam >= 0) {
+        const float s0 = pstage[0][rank], s1 = pstage[1][rank], s2 = pstage[2][rank];
+        const float e0 = u0 - fmaf(J[18], s0, fmaf(J[19], s1, J[20] * s2));
+        const float e1 = u1 - fmaf(J[21], s0, fmaf(J[22], s1, J[23] * s2));
+        dot_part = fmaf(u0, e0, fmaf(u1, e1, dot_part));
+#pragma unroll
+        for (int i = 0; i < 9; ++i) c9[i] = fmaf(J[i], e0, J[9 + i] * e1);
+      }
+#pragma unroll
+      for (int i = 0; i < 9; ++i) cstage[i][tid] = c9[i];
+    }
+    consumer_bar<T>();
+    // phase D: one thread per (camera run, component): fp32 in the tile, one fp64 RED across tiles
+    for (int w = tid; w < 9 * nruns; w += T) {
+      const int u = w / 9, a = w - 9 * u;
+      const int s1 = run_slot[u + 1];
+      float acc = 0.f;
+      for (int sl = run_slot[u]; sl < s1; ++sl) acc += cstage[a][sl];
+      atomicAdd(v.q + 9ll * run_cam[u] + a, (double)acc);
+    }
+    // this warp is done with the stage (phase D read its run table from it)
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(empty + s);
+    if (++s == L.stages) { s = 0; ph ^= 1; }
+  }
+  // p.q of the whole CTA: one fp64 atomic
+  double tot = warp_sum((double)dot_part);
+  if ((tid & 31) == 0) red[tid >> 5] = tot;
+  consumer_bar<T>();
+  if (tid < 32) {
+    tot = tid < T / 32 ? red[tid] : 0.0;
+    tot = warp_sum(tot);
+    if (tid == 0) atomicAdd(&v.pcg->pq, tot);
   }
 }
 
@@ -890,7 +1117,48 @@ static cudaError_t launch_pass(const View& v, int iter, cudaStream_t s) {
 }
 
 cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pass<RHS>(v, 0, s); }
-cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) { return launch_pass<MATVEC>(v, iter, s); }
+
+// The pipelined matvec needs the opt-in shared-memory limit and at least two stages; otherwise (or with
+// CASPAR_BA_PIPELINE=0) the one-block-per-tile kernel is used.
+static int g_smem_optin = -1;
+static int smem_optin() {
+  if (g_smem_optin < 0) {
+    int dev = 0, v = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    g_smem_optin = v;
+  }
+  return g_smem_optin;
+}
+
+bool pipelined_matvec_available(const View& v) {
+  static const bool enabled = [] {
+    const char* e = getenv("CASPAR_BA_PIPELINE");
+    return !(e && e[0] == '0');
+  }();
+  if (!enabled || v.num_tiles == 0 || v.T > 512) return false;
+  const PipeLayout L = pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
+  return L.stages >= 2;
+}
+
+cudaError_t configure_kernels(const View& v) {
+  if (!pipelined_matvec_available(v)) return cudaSuccess;
+  const PipeLayout L = pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
+  if (v.T == 256)
+    return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, L.total);
+  return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, L.total);
+}
+
+cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) {
+  if (!pipelined_matvec_available(v)) return launch_pass<MATVEC>(v, iter, s);
+  const PipeLayout L = pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
+  const int grid = v.num_tiles < v.num_sms ? v.num_tiles : v.num_sms;
+  if (v.T == 256)
+    schur_matvec_pipelined_kernel<256><<<grid, 256 + 32, L.total, s>>>(v, iter, L);
+  else
+    schur_matvec_pipelined_kernel<512><<<grid, 512 + 32, L.total, s>>>(v, iter, L);
+  return CBA_LAUNCHED();
+}
 
 cudaError_t launch_pcg_init(const View& v, cudaStream_t s) {
   if (v.nc == 0) return cudaSuccess;
@@ -953,7 +1221,7 @@ cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* 
   matvec_load_kernel<<<g, 256, 0, s>>>(v, p_in);
   cudaError_t e = CBA_LAUNCHED();
   if (e != cudaSuccess) return e;
-  e = launch_pass<MATVEC>(v, 0, s);
+  e = launch_schur_matvec(v, 0, s);
   if (e != cudaSuccess) return e;
   matvec_finish_kernel<<<g, 256, 0, s>>>(v, q_out);
   return CBA_LAUNCHED();

@@ -156,6 +156,40 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
     out->run_slot[w] = (unsigned short)cnt;
   }
 
+  // --- 3b. per-tile metadata blobs for the TMA-bulk pipelined kernels --------------------------------
+  {
+    auto pad16 = [](size_t bytes) { return (bytes + 15) & ~size_t(15); };
+    std::vector<size_t> off(num_tiles + 1, 0);
+    for (int t = 0; t < num_tiles; ++t) {
+      const int npts = tile_pt[t + 1] - tile_pt[t], nruns = runs_per_tile[t];
+      const size_t bytes = 16 + pad16(2 * (size_t)(npts + 1)) + pad16(2 * (size_t)(nruns + 1)) + pad16(4 * (size_t)nruns);
+      off[t + 1] = off[t] + bytes;
+      out->max_pts_per_tile = std::max(out->max_pts_per_tile, npts);
+      out->meta_max_bytes = std::max(out->meta_max_bytes, (int)bytes);
+    }
+    out->tile_meta.assign(off[num_tiles] ? off[num_tiles] : 16, 0);
+    out->tile_dir.assign(4 * (size_t)(num_tiles ? num_tiles : 1), 0);
+#pragma omp parallel for schedule(static)
+    for (int t = 0; t < num_tiles; ++t) {
+      const int npts = tile_pt[t + 1] - tile_pt[t], nruns = runs_per_tile[t];
+      const int base = out->pt_ptr[tile_pt[t]];
+      unsigned char* blob = out->tile_meta.data() + off[t];
+      int* hdr = reinterpret_cast<int*>(blob);
+      hdr[0] = npts; hdr[1] = nruns; hdr[2] = out->pt_ptr[tile_pt[t + 1]] - base; hdr[3] = tile_pt[t];
+      unsigned short* pt_start = reinterpret_cast<unsigned short*>(blob + 16);
+      for (int a = 0; a <= npts; ++a) pt_start[a] = (unsigned short)(out->pt_ptr[tile_pt[t] + a] - base);
+      unsigned short* rs = reinterpret_cast<unsigned short*>(blob + 16 + pad16(2 * (size_t)(npts + 1)));
+      int* rc = reinterpret_cast<int*>(blob + 16 + pad16(2 * (size_t)(npts + 1)) + pad16(2 * (size_t)(nruns + 1)));
+      const int rb = out->run_begin[t];
+      for (int u = 0; u <= nruns; ++u) rs[u] = out->run_slot[rb + u];
+      for (int u = 0; u < nruns; ++u) rc[u] = out->run_cam[rb + u];
+      out->tile_dir[4 * (size_t)t + 0] = (int)(off[t] / 16);
+      out->tile_dir[4 * (size_t)t + 1] = (int)(off[t + 1] - off[t]);
+      out->tile_dir[4 * (size_t)t + 2] = tile_pt[t];
+      out->tile_dir[4 * (size_t)t + 3] = npts;
+    }
+  }
+
   // --- 4. camera-ordered slot list in chunks ---------------------------------------------------
   std::vector<long long> cptr(nc + 1, 0);
   for (long long i = 0; i < n; ++i) cptr[cam_idx[i] + 1]++;
