@@ -76,6 +76,11 @@ typedef struct {
   caspar_ba_pcg_info pcg;
 } caspar_ba_step_info;
 
+/* Environment (read once per caspar_ba_create; tuning / test switches, not needed in normal use):
+ *   CASPAR_BA_TILE=256|512|1024  force the tile size T (default: chosen from the longest track and N);
+ *   CASPAR_BA_PIPELINE=0         use the one-block-per-tile Schur pass instead of the persistent
+ *                                TMA-pipelined matvec kernel. */
+
 /* Build a solver for one problem: validates the indices, reorders the observations (sorted by point
  * into tiles of whole points, camera runs contiguous inside a tile), carves the arena.
  * Errors: EINVAL (bad sizes / indices / a track longer than CASPAR_BA_MAX_TRACK), ENOMEM, ECUDA. */
@@ -145,6 +150,8 @@ typedef struct {
   /* CUDA-event time of the two dominant kernels, accumulated while profiling is on:              */
   double linearize_ms_total, matvec_ms_total;
   int64_t linearize_count, matvec_count;
+  int32_t matvec_pipelined;  /* 1: the Schur matvec runs as the persistent TMA-pipelined kernel       */
+  int32_t pipeline_stages;   /* shared-memory ring depth of that kernel (0 if not used)               */
 } caspar_ba_stats;
 /* Synchronises the stream the timed kernels ran on, then fills *out. */
 int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out);

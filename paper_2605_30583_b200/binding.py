@@ -49,7 +49,8 @@ class Stats(C.Structure):
     _fields_ = [("tile_slots", C.c_int32), ("num_tiles", C.c_int32), ("padded_slots", C.c_int64),
                 ("camera_runs", C.c_int64), ("arena_bytes", C.c_int64), ("kernels_launched", C.c_int64),
                 ("linearize_ms_total", C.c_double), ("matvec_ms_total", C.c_double),
-                ("linearize_count", C.c_int64), ("matvec_count", C.c_int64)]
+                ("linearize_count", C.c_int64), ("matvec_count", C.c_int64),
+                ("matvec_pipelined", C.c_int32), ("pipeline_stages", C.c_int32)]
 
 
 class LayoutInfo(C.Structure):

@@ -332,6 +332,10 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     v.num_sms = sms > 0 ? sms : 148;
   }
+  {
+    const char* env = std::getenv("CASPAR_BA_PIPELINE");  // "0" selects the one-block-per-tile Schur pass
+    v.pipeline = (!(env && env[0] == '0') && pipelined_matvec_possible(v)) ? 1 : 0;
+  }
   h->camera_runs = ro.camera_runs;
   h->arena_bytes = carve(h, nullptr, ro);
   cudaError_t e = cudaMalloc(&h->arena, h->arena_bytes);
@@ -595,6 +599,8 @@ int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {
   out->matvec_ms_total = h->mv_ms;
   out->linearize_count = h->lin_n;
   out->matvec_count = h->mv_n;
+  out->matvec_pipelined = h->v.pipeline;
+  out->pipeline_stages = h->v.pipeline ? pipeline_stages(h->v) : 0;
   return CASPAR_BA_OK;
 }
 

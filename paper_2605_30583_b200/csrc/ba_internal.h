@@ -88,6 +88,7 @@ struct View {
   const unsigned char* tile_meta;  // blobs
   int max_pts_per_tile, meta_max_bytes;
   int num_sms;
+  int pipeline;                    // 1: Schur matvec runs as the persistent TMA-pipelined kernel
   // per internal point
   const int* pt_ptr;      // [np_obs + 1] prefix sum of track lengths
   const int* pt_perm;     // [np] internal -> caller point id
@@ -157,7 +158,9 @@ cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);
 cudaError_t launch_pcg_init(const View& v, cudaStream_t s);
 cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s);
 cudaError_t configure_kernels(const View& v);  // once per handle: dynamic shared memory opt-in
-bool pipelined_matvec_available(const View& v);
+bool pipelined_matvec_possible(const View& v);   // shape / shared-memory check, at create
+bool pipelined_matvec_available(const View& v);  // = v.pipeline
+int pipeline_stages(const View& v);
 cudaError_t launch_pcg_update(const View& v, int iter, double tol2, cudaStream_t s);  // two kernels
 cudaError_t launch_backsub(const View& v, cudaStream_t s);
 cudaError_t launch_trial_update(const View& v, cudaStream_t s);

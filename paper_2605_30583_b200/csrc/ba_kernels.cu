@@ -1131,14 +1131,15 @@ static int smem_optin() {
   return g_smem_optin;
 }
 
-bool pipelined_matvec_available(const View& v) {
-  static const bool enabled = [] {
-    const char* e = getenv("CASPAR_BA_PIPELINE");
-    return !(e && e[0] == '0');
-  }();
-  if (!enabled || v.num_tiles == 0 || v.T > 512) return false;
+bool pipelined_matvec_possible(const View& v) {
+  if (v.num_tiles == 0 || v.T > 512) return false;
   const PipeLayout L = pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
   return L.stages >= 2;
+}
+
+bool pipelined_matvec_available(const View& v) { return v.pipeline != 0; }
+int pipeline_stages(const View& v) {
+  return pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin()).stages;
 }
 
 cudaError_t configure_kernels(const View& v) {
