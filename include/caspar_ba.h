@@ -101,7 +101,13 @@ int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max
 /* Steps S1-S10: linearize if the cache is stale, pcg_solve, evaluate the trial point x + delta, gain ratio,
  * then commit (parameters updated in place, cache stale) or discard (cache stays valid).
  * accept_mode: 0 = accept iff rho > 0 and the trial cost is finite, 1 = always, 2 = never (dry run).
- * info: HOST, required. */
+ * info: HOST, required.
+ * Linear-solve failures do not abort the iteration: a curvature breakdown
+ * p.Sp <= 0 after at least one iteration truncates PCG at the last good iterate and the step is judged by its
+ * gain ratio; a damped block that is not positive definite in fp32 (or a breakdown before the first iterate)
+ * gives a REJECTED step whatever accept_mode says (accepted = 0, rho = -1, cost_after = cost_before, text in
+ * caspar_ba_last_error), so that the caller's damping update raises lambda.  Errors: ENUMERIC (non-finite
+ * cost at the CURRENT parameters), ECUDA, EINVAL. */
 int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, int32_t accept_mode,
                       void* cuda_stream, caspar_ba_step_info* info);
 

@@ -336,6 +336,7 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
     const char* env = std::getenv("CASPAR_BA_PIPELINE");  // "0" selects the one-block-per-tile Schur pass
     v.pipeline = (!(env && env[0] == '0') && pipelined_matvec_possible(v)) ? 1 : 0;
   }
+  if (const char* env = std::getenv("CASPAR_BA_DEBUG")) v.dbg = std::atoi(env);
   h->camera_runs = ro.camera_runs;
   h->arena_bytes = carve(h, nullptr, ro);
   cudaError_t e = cudaMalloc(&h->arena, h->arena_bytes);
@@ -473,8 +474,25 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
     return fail(h, CASPAR_BA_ENUMERIC, "non-finite cost");
   }
   fill_pcg_info(h, &info->pcg);
-  rc = check_numeric(h);
-  if (rc) return rc;
+  // A curvature breakdown after at least one good iteration truncates the solve at the last good iterate
+  // (Steihaug-style truncated CG): with fp32 Jacobians the computed Schur operator can lose positive
+  // definiteness at lambda ~ 1e-6.  The step is then judged by its gain ratio like any other.
+  if (h->h_pcg->breakdown && h->h_pcg->iters >= 1 && !h->h_step->bad_block) h->h_pcg->breakdown = 0;
+  // A failed linear solve (a damped block that is not positive definite in fp32, or a breakdown before the
+  // first iterate) is a REJECTED step, not an error: parameters and the cached linearization stay, the caller's
+  // damping update raises lambda (what every LM driver does with a failed solve).  accept_mode cannot override
+  // it: there is no step to accept.
+  if (h->h_step->bad_block || h->h_pcg->breakdown) {
+    h->err = h->h_step->bad_block ? "linear solve failed: a damped 9x9 or 3x3 block is not positive definite"
+                                  : "linear solve failed: PCG breakdown before the first iterate";
+    info->cost_before = info->cost_after = h->cost;
+    info->model_decrease = 0.0;
+    info->rho = -1.0;
+    info->accepted = 0;
+    info->pcg.converged = 0;
+    h->have_delta = false;
+    return CASPAR_BA_OK;
+  }
   // S10 gain ratio (host scalars)
   info->cost_before = h->cost;
   info->cost_after = 0.5 * h->h_step->trial_cost;
@@ -483,7 +501,8 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   bool accept;
   if (accept_mode == 1) accept = true;
   else if (accept_mode == 2) accept = false;
-  else accept = std::isfinite(info->cost_after) && info->rho > 0.0;
+  else  // rho > 0 with an actual decrease: a truncated fp32 solve can make BOTH differences negative
+    accept = std::isfinite(info->cost_after) && info->rho > 0.0 && info->cost_after < info->cost_before;
   info->accepted = accept ? 1 : 0;
   if (accept) {
     CK(launch_commit(v, s));

@@ -25,7 +25,7 @@
 
 namespace cba {
 
-constexpr int kCamTableFloats = 28;  // per-camera table row (7 x float4), see camera_prepass_kernel
+constexpr int kCamTableFloats = 36;  // per-camera table row (9 x 16 B: 12 doubles + 12 floats), see camera_prepass_kernel
 constexpr int kCamPad = 12;          // fp32 camera-vector copies (p, delta_c) are padded 9 -> 12 floats
 constexpr int kUg = 54;              // 45 upper-triangle entries of U_j + 9 of g_c,j, fp64 accumulators
 constexpr int kChunkSlots = 1024;    // camera-ordered assembly: slots per work item
@@ -39,6 +39,7 @@ struct PcgScalars {
   double rr;      // |r|^2 after the current update
   double bnorm2;  // |b|^2
   double rz0;
+  double pscale;  // the fp32 direction handed to the matvec is p * pscale (a power of two)
   int done;       // set once converged / broken down: every later kernel returns immediately
   int converged;
   int breakdown;  // p.Sp <= 0 or non-finite
@@ -88,6 +89,7 @@ struct View {
   const unsigned char* tile_meta;  // blobs
   int max_pts_per_tile, meta_max_bytes;
   int num_sms;
+  int dbg;                         // experiment knobs (CASPAR_BA_DEBUG), 0 in production
   int pipeline;                    // 1: Schur matvec runs as the persistent TMA-pipelined kernel
   // per internal point
   const int* pt_ptr;      // [np_obs + 1] prefix sum of track lengths

@@ -79,9 +79,10 @@ __global__ void unpack_points_kernel(View v, const float4* __restrict__ src, flo
 
 // ------------------------------------------------------------------------------------------------
 // S1 camera prepass: everything that depends on the camera alone, once per camera, in fp64.
-// Table row (28 floats): R[9] | C_hi[3] | C_lo[3] | w[3] | f k1 k2 | a b a1 b1 th2 | pad[2]
-// with C = -R^T t the camera centre split into two floats, so that P = R (X - C) is evaluated
-// without the cancellation of R X + t for scenes far from the origin.
+// Table row (144 B = 9 x 16 B):  double R[9] | double C[3] | float f k1 k2 th2 | w0 w1 w2 a | b a1 b1 pad
+// with C = -R^T t the camera centre, so that P = R (X - C) is evaluated without the cancellation of
+// R X + t for scenes far from the origin.  R and C stay in fp64 because the residual is evaluated in
+// fp64 (C12: fp32 cannot resolve uv - pixel to 1e-5 relative); the Jacobian path rounds them.
 // ------------------------------------------------------------------------------------------------
 __global__ void camera_prepass_kernel(int nc, const float* __restrict__ cams, float* __restrict__ table) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
@@ -110,56 +111,62 @@ __global__ void camera_prepass_kernel(int nc, const float* __restrict__ cams, fl
   R[0] = 1.0 + b * (w0 * w0 - th2); R[1] = -a * w2 + b * w0 * w1;     R[2] = a * w1 + b * w0 * w2;
   R[3] = a * w2 + b * w1 * w0;      R[4] = 1.0 + b * (w1 * w1 - th2); R[5] = -a * w0 + b * w1 * w2;
   R[6] = -a * w1 + b * w2 * w0;     R[7] = a * w0 + b * w2 * w1;      R[8] = 1.0 + b * (w2 * w2 - th2);
-  const double C0 = -(R[0] * t0 + R[3] * t1 + R[6] * t2);
-  const double C1 = -(R[1] * t0 + R[4] * t1 + R[7] * t2);
-  const double C2 = -(R[2] * t0 + R[5] * t1 + R[8] * t2);
   float* o = table + (long long)kCamTableFloats * j;
+  double* od = reinterpret_cast<double*>(o);
 #pragma unroll
-  for (int i = 0; i < 9; ++i) o[i] = (float)R[i];
-  const float h0 = (float)C0, h1 = (float)C1, h2 = (float)C2;
-  o[9] = h0; o[10] = h1; o[11] = h2;
-  o[12] = (float)(C0 - (double)h0); o[13] = (float)(C1 - (double)h1); o[14] = (float)(C2 - (double)h2);
-  o[15] = c[0]; o[16] = c[1]; o[17] = c[2];
-  o[18] = c[6]; o[19] = c[7]; o[20] = c[8];
-  o[21] = (float)a; o[22] = (float)b; o[23] = (float)a1; o[24] = (float)b1; o[25] = (float)th2;
-  o[26] = 0.f; o[27] = 0.f;
+  for (int i = 0; i < 9; ++i) od[i] = R[i];
+  od[9] = -(R[0] * t0 + R[3] * t1 + R[6] * t2);
+  od[10] = -(R[1] * t0 + R[4] * t1 + R[7] * t2);
+  od[11] = -(R[2] * t0 + R[5] * t1 + R[8] * t2);
+  o[24] = c[6]; o[25] = c[7]; o[26] = c[8]; o[27] = (float)th2;
+  o[28] = c[0]; o[29] = c[1]; o[30] = c[2]; o[31] = (float)a;
+  o[32] = (float)b; o[33] = (float)a1; o[34] = (float)b1; o[35] = 0.f;
 }
 
 // ------------------------------------------------------------------------------------------------
 // S2 per-observation arithmetic (registers only).  PAPER.md:194-203; O1/O2.
+// The projection and the residual are evaluated in fp64 from the fp64 R, C of the camera table
+// (about 35 fp64 instructions per observation, hidden under the HBM bound); everything the Jacobian
+// needs is rounded to fp32 once.
 // ------------------------------------------------------------------------------------------------
 struct Projection {
   float px, py, n, rad, inz, r0, r1;  // p, |p|^2, radial factor, -1/P_z, residual
+  float R[9];                         // rotation rounded to fp32 (J_p = A R)
 };
 
-__device__ __forceinline__ Projection project(const float4 t0, const float4 t1, const float4 t2, const float4 t3,
-                                              float f, float k1, float k2, float X0, float X1, float X2, float2 m) {
-  // d = X - C (two-float centre), P = R d
-  const float d0 = (X0 - t2.y) - t3.x, d1 = (X1 - t2.z) - t3.y, d2 = (X2 - t2.w) - t3.z;
-  const float P0 = fmaf(t0.x, d0, fmaf(t0.y, d1, t0.z * d2));
-  const float P1 = fmaf(t0.w, d0, fmaf(t1.x, d1, t1.y * d2));
-  const float P2 = fmaf(t1.z, d0, fmaf(t1.w, d1, t2.x * d2));
+__device__ __forceinline__ Projection project(const float4* __restrict__ row, float f, float k1, float k2, float X0,
+                                              float X1, float X2, float2 m) {
+  const double2* rd = reinterpret_cast<const double2*>(row);
+  const double2 a0 = __ldg(rd + 0), a1 = __ldg(rd + 1), a2 = __ldg(rd + 2), a3 = __ldg(rd + 3);
+  const double2 a4 = __ldg(rd + 4), a5 = __ldg(rd + 5);  // R0 R1 | R2 R3 | R4 R5 | R6 R7 | R8 C0 | C1 C2
+  const double d0 = (double)X0 - a4.y, d1 = (double)X1 - a5.x, d2 = (double)X2 - a5.y;
+  const double P0 = fma(a0.x, d0, fma(a0.y, d1, a1.x * d2));
+  const double P1 = fma(a1.y, d0, fma(a2.x, d1, a2.y * d2));
+  const double P2 = fma(a3.x, d0, fma(a3.y, d1, a4.x * d2));
+  const double inz = -1.0 / P2;  // one shared reciprocal
+  const double px = P0 * inz, py = P1 * inz;
+  const double n = fma(px, px, py * py);
+  const double rad = fma(n, fma((double)k2, n, (double)k1), 1.0);
+  const double fr = (double)f * rad;
   Projection o;
-  o.inz = -__frcp_rn(P2);  // one shared reciprocal
-  o.px = P0 * o.inz;
-  o.py = P1 * o.inz;
-  o.n = fmaf(o.px, o.px, o.py * o.py);
-  o.rad = fmaf(o.n, fmaf(k2, o.n, k1), 1.0f);
-  const float fr = f * o.rad;
-  o.r0 = fmaf(fr, o.px, -m.x);
-  o.r1 = fmaf(fr, o.py, -m.y);
+  o.r0 = (float)fma(fr, px, -(double)m.x);
+  o.r1 = (float)fma(fr, py, -(double)m.y);
+  o.px = (float)px; o.py = (float)py; o.n = (float)n; o.rad = (float)rad; o.inz = (float)inz;
+  o.R[0] = (float)a0.x; o.R[1] = (float)a0.y; o.R[2] = (float)a1.x;
+  o.R[3] = (float)a1.y; o.R[4] = (float)a2.x; o.R[5] = (float)a2.y;
+  o.R[6] = (float)a3.x; o.R[7] = (float)a3.y; o.R[8] = (float)a4.x;
   return o;
 }
 
 // Full linearization of one observation: J[0..17] = d r / d camera (2x9 row-major), J[18..23] = d r / d point.
 __device__ __forceinline__ void linearize_observation(const float* __restrict__ table, int cam, float X0, float X1,
                                                       float X2, float2 m, float (&J)[24], float& r0, float& r1) {
-  const float4* row = reinterpret_cast<const float4*>(table) + 7ll * cam;
-  const float4 t0 = __ldg(row + 0), t1 = __ldg(row + 1), t2 = __ldg(row + 2), t3 = __ldg(row + 3);
-  const float4 t4 = __ldg(row + 4), t5 = __ldg(row + 5), t6 = __ldg(row + 6);
-  const float w0 = t3.w, w1 = t4.x, w2 = t4.y, f = t4.z, k1 = t4.w, k2 = t5.x;
-  const float a = t5.y, b = t5.z, a1 = t5.w, b1 = t6.x, th2 = t6.y;
-  const Projection pr = project(t0, t1, t2, t3, f, k1, k2, X0, X1, X2, m);
+  const float4* row = reinterpret_cast<const float4*>(table) + 9ll * cam;
+  const float4 t6 = __ldg(row + 6), t7 = __ldg(row + 7), t8 = __ldg(row + 8);
+  const float f = t6.x, k1 = t6.y, k2 = t6.z, th2 = t6.w;
+  const float w0 = t7.x, w1 = t7.y, w2 = t7.z, a = t7.w;
+  const float b = t8.x, a1 = t8.y, b1 = t8.z;
+  const Projection pr = project(row, f, k1, k2, X0, X1, X2, m);
   r0 = pr.r0;
   r1 = pr.r1;
   const float px = pr.px, py = pr.py, n = pr.n, rad = pr.rad, inz = pr.inz;
@@ -198,20 +205,20 @@ __device__ __forceinline__ void linearize_observation(const float* __restrict__ 
   J[16] = fn * py;
   J[17] = fn * n * py;
   // J_p = A R
-  J[18] = fmaf(A00, t0.x, fmaf(A01, t0.w, A02 * t1.z));
-  J[19] = fmaf(A00, t0.y, fmaf(A01, t1.x, A02 * t1.w));
-  J[20] = fmaf(A00, t0.z, fmaf(A01, t1.y, A02 * t2.x));
-  J[21] = fmaf(A10, t0.x, fmaf(A11, t0.w, A12 * t1.z));
-  J[22] = fmaf(A10, t0.y, fmaf(A11, t1.x, A12 * t1.w));
-  J[23] = fmaf(A10, t0.z, fmaf(A11, t1.y, A12 * t2.x));
+  const float* R = pr.R;
+  J[18] = fmaf(A00, R[0], fmaf(A01, R[3], A02 * R[6]));
+  J[19] = fmaf(A00, R[1], fmaf(A01, R[4], A02 * R[7]));
+  J[20] = fmaf(A00, R[2], fmaf(A01, R[5], A02 * R[8]));
+  J[21] = fmaf(A10, R[0], fmaf(A11, R[3], A12 * R[6]));
+  J[22] = fmaf(A10, R[1], fmaf(A11, R[4], A12 * R[7]));
+  J[23] = fmaf(A10, R[2], fmaf(A11, R[5], A12 * R[8]));
 }
 
 __device__ __forceinline__ void residual_observation(const float* __restrict__ table, int cam, float X0, float X1,
                                                      float X2, float2 m, float& r0, float& r1) {
-  const float4* row = reinterpret_cast<const float4*>(table) + 7ll * cam;
-  const float4 t0 = __ldg(row + 0), t1 = __ldg(row + 1), t2 = __ldg(row + 2), t3 = __ldg(row + 3);
-  const float4 t4 = __ldg(row + 4), t5 = __ldg(row + 5);
-  const Projection pr = project(t0, t1, t2, t3, t4.z, t4.w, t5.x, X0, X1, X2, m);
+  const float4* row = reinterpret_cast<const float4*>(table) + 9ll * cam;
+  const float4 t6 = __ldg(row + 6);
+  const Projection pr = project(row, t6.x, t6.y, t6.z, X0, X1, X2, m);
   r0 = pr.r0;
   r1 = pr.r1;
 }
@@ -512,11 +519,12 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v,
       v.dp[k] = make_float4(s0, s1, s2, 0.f);
       dg_part += fmaf(s0, g.x, fmaf(s1, g.y, s2 * g.z));
     }
+
     for (int r = rb; r < re; ++r) { stage[0][r] = s0; stage[1][r] = s1; stage[2][r] = s2; }
   }
   __syncthreads();
   float c9[9];
-  float dot_part = 0.f;
+  double dot_part = 0.0;  // fp64: squares of fp32 values underflow once |p| falls below ~1e-19
 #pragma unroll
   for (int i = 0; i < 9; ++i) c9[i] = 0.f;
   if (cam >= 0) {
@@ -525,11 +533,11 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v,
     const float w1 = fmaf(J[21], s0, fmaf(J[22], s1, J[23] * s2));
     if (MODE == BACKSUB) {
       const float y0 = u0 + w0, y1 = u1 + w1;  // (J delta)_i
-      dot_part = fmaf(y0, y0, y1 * y1);
+      dot_part = (double)y0 * (double)y0 + (double)y1 * (double)y1;
     } else {
       const float e0 = (MODE == MATVEC) ? u0 - w0 : w0;
       const float e1 = (MODE == MATVEC) ? u1 - w1 : w1;
-      if (MODE == MATVEC) dot_part = fmaf(u0, e0, u1 * e1);
+      if (MODE == MATVEC) dot_part = (double)u0 * (double)e0 + (double)u1 * (double)e1;
 #pragma unroll
       for (int i = 0; i < 9; ++i) c9[i] = fmaf(J[i], e0, J[9 + i] * e1);
     }
@@ -551,11 +559,11 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v,
     }
   }
   if (MODE == MATVEC) {
-    const double tot = block_sum((double)dot_part, red);
+    const double tot = block_sum(dot_part, red);
     if (tid == 0) atomicAdd(&v.pcg->pq, tot);
   }
   if (MODE == BACKSUB) {
-    const double jd2 = block_sum((double)dot_part, red);
+    const double jd2 = block_sum(dot_part, red);
     const double dg = block_sum((double)dg_part, red);
     if (tid == 0) {
       atomicAdd(&v.step->jd2, jd2);
@@ -616,40 +624,50 @@ __device__ __forceinline__ void consumer_bar() {
 
 struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
   int j, cam, rank, vinv, meta, stage_bytes;
-  int stages, pstage, cstage, red, bars, total;
+  int stages, groups, pstage, pstage_bytes, scratch, bars, total;
 };
 
-__host__ __device__ inline PipeLayout pipe_layout(int T, int max_pts, int meta_max, int smem_limit) {
+constexpr int kWarpScratchBytes = 1536;  // per consumer warp: 9 x 33 floats of products + 32 x 2 ints of segments
+
+constexpr int kMaxStages = 8;
+
+// NG consumer groups of T threads share the ring; each group owns a double-buffered point-staging area.
+__host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, int meta_max, int smem_limit) {
   PipeLayout L;
   auto up = [](int x) { return (x + 127) & ~127; };
+  L.groups = NG;
   L.j = 0;
   L.cam = L.j + 6 * T * 16;
   L.rank = L.cam + T * 4;
   L.vinv = up(L.rank + T * 2);
   L.meta = up(L.vinv + max_pts * 32);
   L.stage_bytes = up(L.meta + meta_max);
-  const int fixed = up(3 * (T + 1) * 4) + up(9 * (T + 1) * 4) + 256 + 128;
+  L.pstage_bytes = up(3 * (T + 1) * 4);
+  const int fixed = NG * 2 * L.pstage_bytes + NG * (T / 32) * kWarpScratchBytes + 128;
   int st = (smem_limit - fixed) / L.stage_bytes;
-  L.stages = st > 4 ? 4 : st;
+  L.stages = st > kMaxStages ? kMaxStages : st;
   L.pstage = L.stages * L.stage_bytes;
-  L.cstage = L.pstage + up(3 * (T + 1) * 4);
-  L.red = L.cstage + up(9 * (T + 1) * 4);
-  L.bars = L.red + 256;
+  L.scratch = L.pstage + NG * 2 * L.pstage_bytes;
+  L.bars = L.scratch + NG * (T / 32) * kWarpScratchBytes;
   L.total = L.bars + 128;
   return L;
 }
 
-template <int T>
-__global__ void __launch_bounds__(T + 32, 1) schur_matvec_pipelined_kernel(View v, int iter, PipeLayout L) {
+__device__ __forceinline__ void group_bar(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+template <int T, int NG>
+__global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(View v, int iter, PipeLayout L) {
   extern __shared__ __align__(128) unsigned char smem[];
   if (v.pcg->done) return;
   const int tid = threadIdx.x;
   unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L.bars);
-  unsigned long long* empty = full + 4;
+  unsigned long long* empty = full + kMaxStages;
   if (tid == 0) {
     for (int s = 0; s < L.stages; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(empty + s, T / 32);
+      mbar_init(empty + s, T / 32);  // one group consumes a stage
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     if (blockIdx.x == 0) {  // accumulators of the update that follows this matvec
@@ -662,9 +680,9 @@ __global__ void __launch_bounds__(T + 32, 1) schur_matvec_pipelined_kernel(View 
   __syncthreads();
   const int G = gridDim.x;
 
-  if (tid >= T) {
+  if (tid >= NG * T) {
     // ===== producer warp: one lane issues every copy =====
-    if (tid == T) {
+    if (tid == NG * T) {
       unsigned long long pol_stream, pol_keep;
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
       asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
@@ -693,100 +711,156 @@ __global__ void __launch_bounds__(T + 32, 1) schur_matvec_pipelined_kernel(View 
     return;
   }
 
-  // ===== consumers =====
-  float(*pstage)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.pstage);
-  float(*cstage)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.cstage);
-  double* red = reinterpret_cast<double*>(smem + L.red);
-  float dot_part = 0.f;
-  int s = 0;
-  unsigned ph = 0;
-  for (int t = blockIdx.x; t < v.num_tiles; t += G) {
+  // ===== consumers: group g takes every NG-th tile of this CTA's sequence =====
+  const int g = tid / T, gt = tid - g * T, lane = tid & 31;
+  const int bar_id = 1 + g;
+  // p.q = sum_i u_i.e_i (+ p.lambda D_c p, added by the update kernel): the curvature of the operator AS COMPUTED,
+  // which is what keeps alpha consistent with q (a rewritten, manifestly positive form was tried and made CG
+  // diverge at lambda ~ 1e-5: DESIGN.md "PCG at tiny lambda").  fp64 accumulation.
+  double dot_part = 0.0;
+  int i = g;                    // index in the CTA's tile sequence
+  int s = g % L.stages;         // stage of sequence index i
+  unsigned ph = (unsigned)((g / L.stages) & 1);
+  int buf = 0;
+  for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G, i += NG, buf ^= 1) {
+    float(*pstage)[T + 1] =
+        reinterpret_cast<float(*)[T + 1]>(smem + L.pstage + (size_t)(2 * g + buf) * L.pstage_bytes);
     mbar_wait(full + s, ph);
     const unsigned char* st = smem + (size_t)s * L.stage_bytes;
-    const int4 hdr = *reinterpret_cast<const int4*>(st + L.meta);
-    const int npts = hdr.x, nruns = hdr.y;
+    const int npts = reinterpret_cast<const int*>(st + L.meta)[0];
     const unsigned short* pt_start = reinterpret_cast<const unsigned short*>(st + L.meta + 16);
-    const unsigned short* run_slot = pt_start + ((npts + 1 + 7) & ~7);
-    const int* run_cam = reinterpret_cast<const int*>(run_slot + ((nruns + 1 + 7) & ~7));
-    const int cam = reinterpret_cast<const int*>(st + L.cam)[tid];
-    const unsigned rank = reinterpret_cast<const unsigned short*>(st + L.rank)[tid];
+    const int cam = reinterpret_cast<const int*>(st + L.cam)[gt];
+    const unsigned rank = reinterpret_cast<const unsigned short*>(st + L.rank)[gt];
     // phase A: u = J_c p_j, scatter J_p^T u to the point-major staging rows
     float4 pa = make_float4(0.f, 0.f, 0.f, 0.f), pb = pa, pc = pa;
     if (cam >= 0) {
-      const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
+      const float4* pv = reinterpret_cast<const float4*>(v.p32) + ((v.dbg & 2) ? 0 : 3ll * cam);
       pa = __ldg(pv); pb = __ldg(pv + 1); pc = __ldg(pv + 2);
     }
-    float J[24];
-#pragma unroll
-    for (int c = 0; c < 6; ++c) {
-      const float4 x = reinterpret_cast<const float4*>(st + L.j + c * T * 16)[tid];
-      J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
-    }
     float u0 = 0.f, u1 = 0.f;
-    if (cam >= 0) {
+    float Jp[6];
+    {
+      float J[24];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        const float4 x = reinterpret_cast<const float4*>(st + L.j + c * T * 16)[gt];
+        J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
+      }
       const float pj[9] = {pa.x, pa.y, pa.z, pa.w, pb.x, pb.y, pb.z, pb.w, pc.x};
 #pragma unroll
-      for (int i = 0; i < 9; ++i) {
-        u0 = fmaf(J[i], pj[i], u0);
-        u1 = fmaf(J[9 + i], pj[i], u1);
+      for (int k = 0; k < 9; ++k) {
+        u0 = fmaf(J[k], pj[k], u0);
+        u1 = fmaf(J[9 + k], pj[k], u1);
       }
-      pstage[0][rank] = fmaf(J[18], u0, J[21] * u1);
-      pstage[1][rank] = fmaf(J[19], u0, J[22] * u1);
-      pstage[2][rank] = fmaf(J[20], u0, J[23] * u1);
-    }
-    consumer_bar<T>();
-    // phase B: one thread per point: t_k = sum over its rank range, s_k = V'^-1 t_k, written back in place
-    if (tid < npts) {
-      const int rb = pt_start[tid], re = pt_start[tid + 1];
-      float t0 = 0.f, t1 = 0.f, t2 = 0.f;
-      for (int r = rb; r < re; ++r) { t0 += pstage[0][r]; t1 += pstage[1][r]; t2 += pstage[2][r]; }
-      const float4 vi = reinterpret_cast<const float4*>(st + L.vinv)[2 * tid];
-      const float4 vj = reinterpret_cast<const float4*>(st + L.vinv)[2 * tid + 1];
-      const float s0 = fmaf(vi.x, t0, fmaf(vi.y, t1, vi.z * t2));
-      const float s1 = fmaf(vi.y, t0, fmaf(vi.w, t1, vj.x * t2));
-      const float s2 = fmaf(vi.z, t0, fmaf(vj.x, t1, vj.y * t2));
-      for (int r = rb; r < re; ++r) { pstage[0][r] = s0; pstage[1][r] = s1; pstage[2][r] = s2; }
-    }
-    consumer_bar<T>();
-    // phase C: e = u - J_p s_k, c = J_c^T e into the slot-major (camera-run) staging rows
-    {
-      float c9[9];
 #pragma unroll
-      for (int i = 0; i < 9; ++i) c9[i] = 0.f;
+      for (int k = 0; k < 6; ++k) Jp[k] = J[18 + k];
+    }
+    if (cam >= 0) {
+      pstage[0][rank] = fmaf(Jp[0], u0, Jp[3] * u1);
+      pstage[1][rank] = fmaf(Jp[1], u0, Jp[4] * u1);
+      pstage[2][rank] = fmaf(Jp[2], u0, Jp[5] * u1);
+    }
+    group_bar(bar_id, T);
+    // phase B: three lanes per point (one per component; lanes 30, 31 idle, ten points per warp and pass):
+    // t_k = sum over the point's rank range, s_k = V'^-1 t_k, written back in place
+    {
+      const int lp = lane / 3, c = lane - 3 * lp;
+      for (int k0 = (gt >> 5) * 10; k0 < npts; k0 += (T / 32) * 10) {
+        const int k = k0 + lp;
+        const bool valid = lane < 30 && k < npts;
+        const int rb = valid ? pt_start[k] : 0, re = valid ? pt_start[k + 1] : 0;
+        float t = 0.f;
+        for (int r = rb; r < re; r += 4) {  // four independent loads per round
+          const float a0 = pstage[c][r];
+          const float a1 = r + 1 < re ? pstage[c][r + 1] : 0.f;
+          const float a2 = r + 2 < re ? pstage[c][r + 2] : 0.f;
+          const float a3 = r + 3 < re ? pstage[c][r + 3] : 0.f;
+          t += (a0 + a1) + (a2 + a3);
+        }
+        const int base = lane - c;
+        const float t0 = __shfl_sync(0xffffffffu, t, base), t1 = __shfl_sync(0xffffffffu, t, base + 1),
+                    t2 = __shfl_sync(0xffffffffu, t, base + 2);
+        if (valid) {
+          const float4 vi = reinterpret_cast<const float4*>(st + L.vinv)[2 * k];      // xx xy xz yy
+          const float2 vj = reinterpret_cast<const float2*>(st + L.vinv)[4 * k + 2];  // yz zz
+          const float m0 = c == 0 ? vi.x : (c == 1 ? vi.y : vi.z);
+          const float m1 = c == 0 ? vi.y : (c == 1 ? vi.w : vj.x);
+          const float m2 = c == 0 ? vi.z : (c == 1 ? vj.x : vj.y);
+          const float sc = fmaf(m0, t0, fmaf(m1, t1, m2 * t2));
+          for (int r = rb; r < re; ++r) pstage[c][r] = sc;
+        }
+      }
+    }
+    group_bar(bar_id, T);
+    // phase C: e = u - J_p s_k, c = J_c^T e; the tile's slots are sorted by camera, so a warp holds whole
+    // pieces of camera runs: segmented warp reduction, then one fp64 RED per (warp, camera, component)
+    float c9[9];
+    {
+      float e0 = 0.f, e1 = 0.f;
       if (cam >= 0) {
         const float s0 = pstage[0][rank], s1 = pstage[1][rank], s2 = pstage[2][rank];
-        const float e0 = u0 - fmaf(J[18], s0, fmaf(J[19], s1, J[20] * s2));
-        const float e1 = u1 - fmaf(J[21], s0, fmaf(J[22], s1, J[23] * s2));
-        dot_part = fmaf(u0, e0, fmaf(u1, e1, dot_part));
+        e0 = u0 - fmaf(Jp[0], s0, fmaf(Jp[1], s1, Jp[2] * s2));
+        e1 = u1 - fmaf(Jp[3], s0, fmaf(Jp[4], s1, Jp[5] * s2));
+        dot_part += (double)u0 * (double)e0 + (double)u1 * (double)e1;
+      }
+      float J[20];  // J_c again, from the stage (cheaper than 18 registers held across two barriers)
 #pragma unroll
-        for (int i = 0; i < 9; ++i) c9[i] = fmaf(J[i], e0, J[9 + i] * e1);
+      for (int c = 0; c < 5; ++c) {
+        const float4 x = reinterpret_cast<const float4*>(st + L.j + c * T * 16)[gt];
+        J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
       }
 #pragma unroll
-      for (int i = 0; i < 9; ++i) cstage[i][tid] = c9[i];
+      for (int k = 0; k < 9; ++k) c9[k] = fmaf(J[k], e0, J[9 + k] * e1);
     }
-    consumer_bar<T>();
-    // phase D: one thread per (camera run, component): fp32 in the tile, one fp64 RED across tiles
-    for (int w = tid; w < 9 * nruns; w += T) {
-      const int u = w / 9, a = w - 9 * u;
-      const int s1 = run_slot[u + 1];
-      float acc = 0.f;
-      for (int sl = run_slot[u]; sl < s1; ++sl) acc += cstage[a][sl];
-      atomicAdd(v.q + 9ll * run_cam[u] + a, (double)acc);
-    }
-    // this warp is done with the stage (phase D read its run table from it)
+    // this warp is done with the stage
     __syncwarp();
-    if ((tid & 31) == 0) mbar_arrive(empty + s);
-    if (++s == L.stages) { s = 0; ph ^= 1; }
+    if (lane == 0) mbar_arrive(empty + s);
+    // Camera side, warp-local: the tile's slots are sorted by camera, so a warp holds whole pieces of camera
+    // runs (lane intervals).  The nine products go to the warp's scratch rows (bank = component + lane:
+    // conflict free), then lane l sums component l % 9 of segment l / 9 and issues one fp64 RED, so that
+    // one instruction covers whole 72-byte camera rows of q.
+    {
+      float* rows = reinterpret_cast<float*>(smem + L.scratch + (size_t)(tid >> 5) * kWarpScratchBytes);
+      int* seg = reinterpret_cast<int*>(rows + 9 * 33);  // (start | end << 8, camera) per segment
+      const int cam_prev = __shfl_up_sync(0xffffffffu, cam, 1);
+      const bool bound = lane == 0 || cam_prev != cam;
+      const unsigned bmask = __ballot_sync(0xffffffffu, bound);
+      const int nseg = __popc(bmask);
+#pragma unroll
+      for (int k = 0; k < 9; ++k) rows[k * 33 + lane] = c9[k];
+      if (bound) {
+        const unsigned later = bmask & ~((2u << lane) - 1u);
+        const int end = later ? __ffs(later) - 1 : 32;
+        const int h = __popc(bmask & ((1u << lane) - 1u));
+        seg[2 * h] = lane | (end << 8);
+        seg[2 * h + 1] = cam;
+      }
+      __syncwarp();
+      if (!(v.dbg & 1))
+      for (int idx = lane; idx < 9 * nseg; idx += 32) {
+        const int h = idx / 9, k = idx - 9 * h;
+        const int se = seg[2 * h], cm = seg[2 * h + 1];
+        const float* src = rows + k * 33;
+        const int end = se >> 8;
+        float acc = 0.f;
+        for (int sl = se & 255; sl < end; sl += 4) {  // four independent loads per round
+          const float a0 = src[sl];
+          const float a1 = sl + 1 < end ? src[sl + 1] : 0.f;
+          const float a2 = sl + 2 < end ? src[sl + 2] : 0.f;
+          const float a3 = sl + 3 < end ? src[sl + 3] : 0.f;
+          acc += (a0 + a1) + (a2 + a3);
+        }
+        if (cm >= 0) atomicAdd(v.q + 9ll * cm + k, (double)acc);
+      }
+      __syncwarp();  // the scratch rows are rewritten by this warp's next tile
+    }
+    // advance to sequence index i + NG
+    s += NG;
+    while (s >= L.stages) { s -= L.stages; ph ^= 1; }
   }
-  // p.q of the whole CTA: one fp64 atomic
-  double tot = warp_sum((double)dot_part);
-  if ((tid & 31) == 0) red[tid >> 5] = tot;
-  consumer_bar<T>();
-  if (tid < 32) {
-    tot = tid < T / 32 ? red[tid] : 0.0;
-    tot = warp_sum(tot);
-    if (tid == 0) atomicAdd(&v.pcg->pq, tot);
-  }
+  // p.q: one fp64 atomic per warp
+  const double tot = warp_sum(dot_part);
+  if (lane == 0) atomicAdd(&v.pcg->pq, tot);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -802,7 +876,26 @@ __device__ __forceinline__ double apply_minv(const View& v, int j, int a, const 
   return z;
 }
 
-// x = 0, r = b, z = M^-1 r, p = z; rz[0], |b|^2, pDp[0]
+// The fp32 copy of the search direction is p * 2^-e with 2^e ~ |r|: the matvec then works at O(1)
+// magnitudes whatever the residual has shrunk to (fp32 products of a direction below ~1e-19 would
+// underflow), and q, p.q are scaled back exactly (powers of two) by the update kernel.
+__device__ __forceinline__ double direction_scale(double rr) {
+  if (!(rr > 0.0) || !isfinite(rr)) return 1.0;
+  int e;
+  frexp(rr, &e);
+  return ldexp(1.0, -(e / 2));
+}
+
+// |b|^2, needed before the first direction is rounded to fp32
+__global__ void __launch_bounds__(kPcgThreads) pcg_norm_kernel(View v) {
+  __shared__ double red[32];
+  const long long i = (long long)blockIdx.x * kPcgThreads + threadIdx.x;
+  const double bi = i < 9ll * v.nc ? v.b[i] : 0.0;
+  const double s = block_sum(bi * bi, red);
+  if (threadIdx.x == 0) atomicAdd(&v.pcg->bnorm2, s);
+}
+
+// x = 0, r = b, z = M^-1 r, p = z; rz[0], |r|^2, pDp[0]
 __global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v) {
   __shared__ double rs[kPcgThreads];
   __shared__ double red[32];
@@ -813,6 +906,7 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v) {
   const double ri = valid ? v.b[i] : 0.0;
   rs[tid] = ri;
   __syncthreads();
+  const double scale = direction_scale(v.pcg->bnorm2);
   double zi = 0.0, ld = 0.0;
   if (valid) {
     zi = apply_minv(v, j, a, rs + (tid - a));
@@ -822,16 +916,16 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v) {
     v.z[i] = zi;
     v.p[i] = zi;
     v.q[i] = 0.0;
-    v.p32[(long long)kCamPad * j + a] = (float)zi;
+    v.p32[(long long)kCamPad * j + a] = (float)(zi * scale);
   }
   const double s_rz = block_sum(ri * zi, red);
   const double s_rr = block_sum(ri * ri, red);
   const double s_pd = block_sum(ld * zi * zi, red);
   if (tid == 0) {
     atomicAdd(&v.pcg->rz[0], s_rz);
-    atomicAdd(&v.pcg->bnorm2, s_rr);
     atomicAdd(&v.pcg->rr, s_rr);
     atomicAdd(&v.pcg->pDp[0], s_pd);
+    if (blockIdx.x == 0) v.pcg->pscale = scale;
   }
 }
 
@@ -842,7 +936,8 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_xr_kernel(View v, int 
   PcgScalars* sc = v.pcg;
   if (sc->done) return;
   const int tid = threadIdx.x, par = iter & 1;
-  const double denom = sc->pq + sc->pDp[par];
+  const double unscale = 1.0 / sc->pscale;  // q and p.q were computed from p * pscale
+  const double denom = sc->pq * unscale * unscale + sc->pDp[par];
   const double rz = sc->rz[par];
   if (!(denom > 0.0) || !isfinite(denom) || !isfinite(rz)) {  // breakdown (C15) or b = 0
     if (blockIdx.x == 0 && tid == 0) {
@@ -858,7 +953,7 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_xr_kernel(View v, int 
   double ri = 0.0;
   if (valid) {
     const double pi = v.p[i];
-    const double qi = v.q[i] + v.lamD[i] * pi;
+    const double qi = v.q[i] * unscale + v.lamD[i] * pi;
     v.x[i] += alpha * pi;
     ri = v.r[i] - alpha * qi;
     v.r[i] = ri;
@@ -893,6 +988,7 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v, int i
     return;
   }
   const double beta = sc->rz[par ^ 1] / sc->rz[par];
+  const double scale = direction_scale(sc->rr);
   const long long i = (long long)blockIdx.x * kPcgThreads + tid;
   const int j = (int)(i / 9), a = (int)(i - 9ll * j);
   double pd = 0.0;
@@ -900,13 +996,16 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v, int i
     const double pi = v.z[i] + beta * v.p[i];
     v.p[i] = pi;
     v.q[i] = 0.0;
-    v.p32[(long long)kCamPad * j + a] = (float)pi;
+    v.p32[(long long)kCamPad * j + a] = (float)(pi * scale);
     pd = v.lamD[i] * pi * pi;
   }
   const double s_pd = block_sum(pd, red);
   if (tid == 0) {
     atomicAdd(&sc->pDp[par ^ 1], s_pd);
-    if (blockIdx.x == 0) sc->pq = 0.0;
+    if (blockIdx.x == 0) {
+      sc->pq = 0.0;
+      sc->pscale = scale;
+    }
   }
 }
 
@@ -1131,38 +1230,46 @@ static int smem_optin() {
   return g_smem_optin;
 }
 
+// Consumer groups per CTA: tiles of 256 slots leave room for three groups (800 threads, <= 80 registers),
+// tiles of 512 for one.
+static int pipe_groups(int T) { return T == 256 ? 3 : 1; }
+
 bool pipelined_matvec_possible(const View& v) {
   if (v.num_tiles == 0 || v.T > 512) return false;
-  const PipeLayout L = pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
+  const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
   return L.stages >= 2;
 }
 
 bool pipelined_matvec_available(const View& v) { return v.pipeline != 0; }
 int pipeline_stages(const View& v) {
-  return pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin()).stages;
+  return pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin()).stages;
 }
 
+// The opt-in limit itself is requested (not this handle's own size): the attribute is per function, and
+// handles with different layouts share the kernel.
 cudaError_t configure_kernels(const View& v) {
   if (!pipelined_matvec_available(v)) return cudaSuccess;
-  const PipeLayout L = pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
   if (v.T == 256)
-    return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, L.total);
-  return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, L.total);
+    return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+  return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
 }
 
 cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) {
   if (!pipelined_matvec_available(v)) return launch_pass<MATVEC>(v, iter, s);
-  const PipeLayout L = pipe_layout(v.T, v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
+  const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
   const int grid = v.num_tiles < v.num_sms ? v.num_tiles : v.num_sms;
   if (v.T == 256)
-    schur_matvec_pipelined_kernel<256><<<grid, 256 + 32, L.total, s>>>(v, iter, L);
+    schur_matvec_pipelined_kernel<256, 3><<<grid, 3 * 256 + 32, L.total, s>>>(v, iter, L);
   else
-    schur_matvec_pipelined_kernel<512><<<grid, 512 + 32, L.total, s>>>(v, iter, L);
+    schur_matvec_pipelined_kernel<512, 1><<<grid, 512 + 32, L.total, s>>>(v, iter, L);
   return CBA_LAUNCHED();
 }
 
 cudaError_t launch_pcg_init(const View& v, cudaStream_t s) {
   if (v.nc == 0) return cudaSuccess;
+  pcg_norm_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
+  cudaError_t e = CBA_LAUNCHED();
+  if (e != cudaSuccess) return e;
   pcg_init_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
   return CBA_LAUNCHED();
 }
