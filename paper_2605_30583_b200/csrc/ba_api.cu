@@ -85,6 +85,7 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.cam = c.take<int>(S);
   v.obs_of_slot = c.take<int>(S);
   v.rank = c.take<unsigned short>(S);
+  v.rankpid = c.take<unsigned short>(ro.rankpid.size());
   v.tile_pt = c.take<int>(ro.tile_pt.size());
   v.run_begin = c.take<int>(ro.run_begin.size());
   v.run_cam = c.take<int>(ro.run_cam.size());
@@ -346,6 +347,7 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   if (e == cudaSuccess) e = upload(v.cam, ro.cam, s);
   if (e == cudaSuccess) e = upload(v.obs_of_slot, ro.obs_of_slot, s);
   if (e == cudaSuccess) e = upload(v.rank, ro.rank, s);
+  if (e == cudaSuccess) e = upload(v.rankpid, ro.rankpid, s);
   if (e == cudaSuccess) e = upload(v.tile_pt, ro.tile_pt, s);
   if (e == cudaSuccess) e = upload(v.run_begin, ro.run_begin, s);
   if (e == cudaSuccess) e = upload(v.run_cam, ro.run_cam, s);

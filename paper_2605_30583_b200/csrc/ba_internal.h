@@ -72,6 +72,7 @@ struct View {
   const float2* px;
   const int* cam;
   const unsigned short* rank;
+  const unsigned short* rankpid;  // rank | local point id << 8 (T <= 256), read by the pipelined matvec
   const int* obs_of_slot;  // caller observation id of a slot (-1 = padding)
   float4* J[6];
   float2* res;
@@ -130,6 +131,7 @@ struct Reordered {
   std::vector<int> obs_of_slot;           // [n_slots]
   std::vector<int> cam;                   // [n_slots]
   std::vector<unsigned short> rank;       // [n_slots]
+  std::vector<unsigned short> rankpid;    // [n_slots] rank | local point id << 8 (tiles of <= 256 slots only)
   std::vector<int> tile_pt;               // [num_tiles + 1]
   std::vector<int> run_begin;             // [num_tiles + 1]
   std::vector<int> run_cam;

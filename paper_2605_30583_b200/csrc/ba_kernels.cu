@@ -223,7 +223,7 @@ __device__ __forceinline__ void residual_observation(const float* __restrict__ t
   r1 = pr.r1;
 }
 
-constexpr int blocks_per_sm(int T) { return T == 256 ? 3 : (T == 512 ? 2 : 1); }
+constexpr int blocks_per_sm(int T) { return T == 128 ? 6 : (T == 256 ? 3 : (T == 512 ? 2 : 1)); }
 
 // ------------------------------------------------------------------------------------------------
 // S2 + S3 (JAC = true): linearize every observation, store r and J, assemble V_k and g_p,k per point,
@@ -624,14 +624,14 @@ __device__ __forceinline__ void consumer_bar() {
 
 struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
   int j, cam, rank, vinv, meta, stage_bytes;
-  int stages, groups, pstage, pstage_bytes, scratch, bars, total;
+  int stages, groups, tbuf, tbuf_bytes, sbuf, sbuf_bytes, scratch, bars, total;
 };
 
-constexpr int kWarpScratchBytes = 1536;  // per consumer warp: 9 x 33 floats of products + 32 x 2 ints of segments
+constexpr int kMaxStages = 12;
+constexpr int kWarpScratchBytes = 1408;  // per consumer warp: 9 x 33 floats of products + 32 camera ids
 
-constexpr int kMaxStages = 8;
-
-// NG consumer groups of T threads share the ring; each group owns a double-buffered point-staging area.
+// NG consumer groups of T threads share the ring; each group owns a staging area for the point-side sums
+// t_k (by rank) and one for the per-point results s_k (by local point id).
 __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, int meta_max, int smem_limit) {
   PipeLayout L;
   auto up = [](int x) { return (x + 127) & ~127; };
@@ -642,14 +642,16 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   L.vinv = up(L.rank + T * 2);
   L.meta = up(L.vinv + max_pts * 32);
   L.stage_bytes = up(L.meta + meta_max);
-  L.pstage_bytes = up(3 * (T + 1) * 4);
-  const int fixed = NG * 2 * L.pstage_bytes + NG * (T / 32) * kWarpScratchBytes + 128;
+  L.tbuf_bytes = up(3 * (T + 1) * 4);
+  L.sbuf_bytes = up(3 * (T + 1) * 4);
+  const int fixed = NG * (L.tbuf_bytes + L.sbuf_bytes) + NG * (T / 32) * kWarpScratchBytes + 256;
   int st = (smem_limit - fixed) / L.stage_bytes;
   L.stages = st > kMaxStages ? kMaxStages : st;
-  L.pstage = L.stages * L.stage_bytes;
-  L.scratch = L.pstage + NG * 2 * L.pstage_bytes;
+  L.tbuf = L.stages * L.stage_bytes;
+  L.sbuf = L.tbuf + NG * L.tbuf_bytes;
+  L.scratch = L.sbuf + NG * L.sbuf_bytes;
   L.bars = L.scratch + NG * (T / 32) * kWarpScratchBytes;
-  L.total = L.bars + 128;
+  L.total = L.bars + 256;
   return L;
 }
 
@@ -701,7 +703,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
 #pragma unroll
         for (int c = 0; c < 6; ++c) bulk_g2s(st + L.j + c * T * 16, v.J[c] + slot0, T * 16, full + s, pol_stream);
         bulk_g2s(st + L.cam, v.cam + slot0, T * 4, full + s, pol_stream);
-        bulk_g2s(st + L.rank, v.rank + slot0, T * 2, full + s, pol_stream);
+        bulk_g2s(st + L.rank, v.rankpid + slot0, T * 2, full + s, pol_stream);
         bulk_g2s(st + L.vinv, v.Vinv + 2ll * d.z, vinv_bytes, full + s, pol_keep);
         bulk_g2s(st + L.meta, v.tile_meta + 16ll * d.x, (unsigned)d.y, full + s, pol_stream);
         d = dn;
@@ -714,27 +716,28 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   // ===== consumers: group g takes every NG-th tile of this CTA's sequence =====
   const int g = tid / T, gt = tid - g * T, lane = tid & 31;
   const int bar_id = 1 + g;
+  float(*tbuf)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.tbuf + (size_t)g * L.tbuf_bytes);  // by rank
+  float(*sbuf)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // by point
+  float* rows = reinterpret_cast<float*>(smem + L.scratch + (size_t)(tid >> 5) * kWarpScratchBytes);
+  int* camrow = reinterpret_cast<int*>(rows + 9 * 33);
   // p.q = sum_i u_i.e_i (+ p.lambda D_c p, added by the update kernel): the curvature of the operator AS COMPUTED,
   // which is what keeps alpha consistent with q (a rewritten, manifestly positive form was tried and made CG
   // diverge at lambda ~ 1e-5: DESIGN.md "PCG at tiny lambda").  fp64 accumulation.
   double dot_part = 0.0;
-  int i = g;                    // index in the CTA's tile sequence
-  int s = g % L.stages;         // stage of sequence index i
+  int s = g % L.stages;  // stage of this group's current tile
   unsigned ph = (unsigned)((g / L.stages) & 1);
-  int buf = 0;
-  for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G, i += NG, buf ^= 1) {
-    float(*pstage)[T + 1] =
-        reinterpret_cast<float(*)[T + 1]>(smem + L.pstage + (size_t)(2 * g + buf) * L.pstage_bytes);
+  for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G) {
     mbar_wait(full + s, ph);
     const unsigned char* st = smem + (size_t)s * L.stage_bytes;
     const int npts = reinterpret_cast<const int*>(st + L.meta)[0];
     const unsigned short* pt_start = reinterpret_cast<const unsigned short*>(st + L.meta + 16);
     const int cam = reinterpret_cast<const int*>(st + L.cam)[gt];
-    const unsigned rank = reinterpret_cast<const unsigned short*>(st + L.rank)[gt];
-    // phase A: u = J_c p_j, scatter J_p^T u to the point-major staging rows
+    const unsigned rp = reinterpret_cast<const unsigned short*>(st + L.rank)[gt];
+    const unsigned rank = rp & 255u, pid = rp >> 8;
+    // ---- phase A: u = J_c p_j, scatter J_p^T u to the point-major staging rows
     float4 pa = make_float4(0.f, 0.f, 0.f, 0.f), pb = pa, pc = pa;
     if (cam >= 0) {
-      const float4* pv = reinterpret_cast<const float4*>(v.p32) + ((v.dbg & 2) ? 0 : 3ll * cam);
+      const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
       pa = __ldg(pv); pb = __ldg(pv + 1); pc = __ldg(pv + 2);
     }
     float u0 = 0.f, u1 = 0.f;
@@ -756,49 +759,48 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       for (int k = 0; k < 6; ++k) Jp[k] = J[18 + k];
     }
     if (cam >= 0) {
-      pstage[0][rank] = fmaf(Jp[0], u0, Jp[3] * u1);
-      pstage[1][rank] = fmaf(Jp[1], u0, Jp[4] * u1);
-      pstage[2][rank] = fmaf(Jp[2], u0, Jp[5] * u1);
+      tbuf[0][rank] = fmaf(Jp[0], u0, Jp[3] * u1);
+      tbuf[1][rank] = fmaf(Jp[1], u0, Jp[4] * u1);
+      tbuf[2][rank] = fmaf(Jp[2], u0, Jp[5] * u1);
     }
     group_bar(bar_id, T);
-    // phase B: three lanes per point (one per component; lanes 30, 31 idle, ten points per warp and pass):
-    // t_k = sum over the point's rank range, s_k = V'^-1 t_k, written back in place
+    // ---- phase B: six lanes per point (component x half of the track; lanes 30, 31 idle, five points per
+    // warp and pass): t_k = sum over the point's rank range, s_k = V'^-1 t_k, stored once per point
     {
-      const int lp = lane / 3, c = lane - 3 * lp;
-      for (int k0 = (gt >> 5) * 10; k0 < npts; k0 += (T / 32) * 10) {
+      const int lp = lane / 6, c = (lane - 6 * lp) >> 1, half = lane & 1;
+      for (int k0 = (gt >> 5) * 5; k0 < npts; k0 += (T / 32) * 5) {
         const int k = k0 + lp;
         const bool valid = lane < 30 && k < npts;
         const int rb = valid ? pt_start[k] : 0, re = valid ? pt_start[k + 1] : 0;
-        float t = 0.f;
-        for (int r = rb; r < re; r += 4) {  // four independent loads per round
-          const float a0 = pstage[c][r];
-          const float a1 = r + 1 < re ? pstage[c][r + 1] : 0.f;
-          const float a2 = r + 2 < re ? pstage[c][r + 2] : 0.f;
-          const float a3 = r + 3 < re ? pstage[c][r + 3] : 0.f;
-          t += (a0 + a1) + (a2 + a3);
+        float tsum = 0.f;
+        for (int r = rb + half; r < re; r += 8) {  // four independent loads per round
+          const float a0 = tbuf[c][r];
+          const float a1 = r + 2 < re ? tbuf[c][r + 2] : 0.f;
+          const float a2 = r + 4 < re ? tbuf[c][r + 4] : 0.f;
+          const float a3 = r + 6 < re ? tbuf[c][r + 6] : 0.f;
+          tsum += (a0 + a1) + (a2 + a3);
         }
-        const int base = lane - c;
-        const float t0 = __shfl_sync(0xffffffffu, t, base), t1 = __shfl_sync(0xffffffffu, t, base + 1),
-                    t2 = __shfl_sync(0xffffffffu, t, base + 2);
-        if (valid) {
+        tsum += __shfl_xor_sync(0xffffffffu, tsum, 1);
+        const int base = 6 * lp;
+        const float t0 = __shfl_sync(0xffffffffu, tsum, base), t1 = __shfl_sync(0xffffffffu, tsum, base + 2),
+                    t2 = __shfl_sync(0xffffffffu, tsum, base + 4);
+        if (valid && half == 0) {
           const float4 vi = reinterpret_cast<const float4*>(st + L.vinv)[2 * k];      // xx xy xz yy
           const float2 vj = reinterpret_cast<const float2*>(st + L.vinv)[4 * k + 2];  // yz zz
           const float m0 = c == 0 ? vi.x : (c == 1 ? vi.y : vi.z);
           const float m1 = c == 0 ? vi.y : (c == 1 ? vi.w : vj.x);
           const float m2 = c == 0 ? vi.z : (c == 1 ? vj.x : vj.y);
-          const float sc = fmaf(m0, t0, fmaf(m1, t1, m2 * t2));
-          for (int r = rb; r < re; ++r) pstage[c][r] = sc;
+          sbuf[c][k] = fmaf(m0, t0, fmaf(m1, t1, m2 * t2));
         }
       }
     }
     group_bar(bar_id, T);
-    // phase C: e = u - J_p s_k, c = J_c^T e; the tile's slots are sorted by camera, so a warp holds whole
-    // pieces of camera runs: segmented warp reduction, then one fp64 RED per (warp, camera, component)
+    // ---- phase C: e = u - J_p s_k, c = J_c^T e
     float c9[9];
     {
       float e0 = 0.f, e1 = 0.f;
       if (cam >= 0) {
-        const float s0 = pstage[0][rank], s1 = pstage[1][rank], s2 = pstage[2][rank];
+        const float s0 = sbuf[0][pid], s1 = sbuf[1][pid], s2 = sbuf[2][pid];
         e0 = u0 - fmaf(Jp[0], s0, fmaf(Jp[1], s1, Jp[2] * s2));
         e1 = u1 - fmaf(Jp[3], s0, fmaf(Jp[4], s1, Jp[5] * s2));
         dot_part += (double)u0 * (double)e0 + (double)u1 * (double)e1;
@@ -815,46 +817,42 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     // this warp is done with the stage
     __syncwarp();
     if (lane == 0) mbar_arrive(empty + s);
-    // Camera side, warp-local: the tile's slots are sorted by camera, so a warp holds whole pieces of camera
-    // runs (lane intervals).  The nine products go to the warp's scratch rows (bank = component + lane:
-    // conflict free), then lane l sums component l % 9 of segment l / 9 and issues one fp64 RED, so that
-    // one instruction covers whole 72-byte camera rows of q.
+    // ---- camera side, warp-local.  The tile's slots are sorted by camera, so a warp holds whole pieces of
+    // camera runs (lane intervals).  The nine products go to the warp's scratch rows (bank = component + lane:
+    // conflict free); lane (k, part) then walks component k over slots [11 part, 11 part + 11) and adds a
+    // partial sum to q at every segment end: the nine lanes of a part act in lockstep, so one fp64 RED
+    // instruction covers a whole 72-byte camera row.  A segment that crosses a part boundary is added in
+    // two pieces.
     {
-      float* rows = reinterpret_cast<float*>(smem + L.scratch + (size_t)(tid >> 5) * kWarpScratchBytes);
-      int* seg = reinterpret_cast<int*>(rows + 9 * 33);  // (start | end << 8, camera) per segment
       const int cam_prev = __shfl_up_sync(0xffffffffu, cam, 1);
-      const bool bound = lane == 0 || cam_prev != cam;
-      const unsigned bmask = __ballot_sync(0xffffffffu, bound);
-      const int nseg = __popc(bmask);
+      const unsigned bmask = __ballot_sync(0xffffffffu, lane == 0 || cam_prev != cam);
 #pragma unroll
       for (int k = 0; k < 9; ++k) rows[k * 33 + lane] = c9[k];
-      if (bound) {
-        const unsigned later = bmask & ~((2u << lane) - 1u);
-        const int end = later ? __ffs(later) - 1 : 32;
-        const int h = __popc(bmask & ((1u << lane) - 1u));
-        seg[2 * h] = lane | (end << 8);
-        seg[2 * h + 1] = cam;
-      }
+      camrow[lane] = cam;
       __syncwarp();
-      if (!(v.dbg & 1))
-      for (int idx = lane; idx < 9 * nseg; idx += 32) {
-        const int h = idx / 9, k = idx - 9 * h;
-        const int se = seg[2 * h], cm = seg[2 * h + 1];
-        const float* src = rows + k * 33;
-        const int end = se >> 8;
+      if (lane < 27 && !(v.dbg & 1)) {
+        const int part = lane / 9, k = lane - 9 * part, s0 = 11 * part;
+        const float* src = rows + k * 33 + s0;
+        // bit i: slot s0 + i is the last slot of a segment (the next slot starts one), or of this part
+        unsigned endm = ((bmask >> 1) | 0x80000000u) >> s0;
+        endm |= part == 2 ? (1u << 9) : (1u << 10);
+        float val[11];
+#pragma unroll
+        for (int i = 0; i < 11; ++i) val[i] = (i < 10 || part < 2) ? src[i] : 0.f;
         float acc = 0.f;
-        for (int sl = se & 255; sl < end; sl += 4) {  // four independent loads per round
-          const float a0 = src[sl];
-          const float a1 = sl + 1 < end ? src[sl + 1] : 0.f;
-          const float a2 = sl + 2 < end ? src[sl + 2] : 0.f;
-          const float a3 = sl + 3 < end ? src[sl + 3] : 0.f;
-          acc += (a0 + a1) + (a2 + a3);
+        double* qk = v.q + k;
+#pragma unroll
+        for (int i = 0; i < 11; ++i) {
+          acc += val[i];
+          if (endm & (1u << i)) {
+            const int cm = camrow[s0 + i];
+            if (cm >= 0) atomicAdd(qk + 9ll * cm, (double)acc);
+            acc = 0.f;
+          }
         }
-        if (cm >= 0) atomicAdd(v.q + 9ll * cm + k, (double)acc);
       }
       __syncwarp();  // the scratch rows are rewritten by this warp's next tile
     }
-    // advance to sequence index i + NG
     s += NG;
     while (s >= L.stages) { s -= L.stages; ph ^= 1; }
   }
@@ -1170,6 +1168,7 @@ static cudaError_t launch_linearize_t(const View& v, const float4* pts, const fl
                                       cudaStream_t s) {
   if (v.num_tiles == 0) return cudaSuccess;
   switch (v.T) {
+    case 128: linearize_kernel<128, JAC><<<v.num_tiles, 128, 0, s>>>(v, pts, table, acc); break;
     case 256: linearize_kernel<256, JAC><<<v.num_tiles, 256, 0, s>>>(v, pts, table, acc); break;
     case 512: linearize_kernel<512, JAC><<<v.num_tiles, 512, 0, s>>>(v, pts, table, acc); break;
     default: linearize_kernel<1024, JAC><<<v.num_tiles, 1024, 0, s>>>(v, pts, table, acc); break;
@@ -1208,6 +1207,7 @@ template <int MODE>
 static cudaError_t launch_pass(const View& v, int iter, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaSuccess;
   switch (v.T) {
+    case 128: schur_pass_kernel<128, MODE><<<v.num_tiles, 128, 0, s>>>(v, iter); break;
     case 256: schur_pass_kernel<256, MODE><<<v.num_tiles, 256, 0, s>>>(v, iter); break;
     case 512: schur_pass_kernel<512, MODE><<<v.num_tiles, 512, 0, s>>>(v, iter); break;
     default: schur_pass_kernel<1024, MODE><<<v.num_tiles, 1024, 0, s>>>(v, iter); break;
@@ -1230,14 +1230,14 @@ static int smem_optin() {
   return g_smem_optin;
 }
 
-// Consumer groups per CTA: tiles of 256 slots leave room for three groups (800 threads, <= 80 registers),
-// tiles of 512 for one.
-static int pipe_groups(int T) { return T == 256 ? 3 : 1; }
+// The pipelined matvec packs rank and local point id into 16 bits, so it serves tiles of <= 256 slots:
+// T = 256 with three consumer groups (800 threads) or T = 128 with six.  Longer tracks use schur_pass_kernel.
+static int pipe_groups(int T) { return T == 256 ? 3 : 6; }
 
 bool pipelined_matvec_possible(const View& v) {
-  if (v.num_tiles == 0 || v.T > 512) return false;
+  if (v.num_tiles == 0 || v.T > 256) return false;
   const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
-  return L.stages >= 2;
+  return L.stages >= pipe_groups(v.T) + 1;
 }
 
 bool pipelined_matvec_available(const View& v) { return v.pipeline != 0; }
@@ -1251,7 +1251,7 @@ cudaError_t configure_kernels(const View& v) {
   if (!pipelined_matvec_available(v)) return cudaSuccess;
   if (v.T == 256)
     return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
-  return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+  return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
 }
 
 cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) {
@@ -1261,7 +1261,7 @@ cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) {
   if (v.T == 256)
     schur_matvec_pipelined_kernel<256, 3><<<grid, 3 * 256 + 32, L.total, s>>>(v, iter, L);
   else
-    schur_matvec_pipelined_kernel<512, 1><<<grid, 512 + 32, L.total, s>>>(v, iter, L);
+    schur_matvec_pipelined_kernel<128, 6><<<grid, 6 * 128 + 32, L.total, s>>>(v, iter, L);
   return CBA_LAUNCHED();
 }
 

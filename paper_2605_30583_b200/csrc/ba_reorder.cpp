@@ -45,10 +45,10 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
     return CASPAR_BA_EINVAL;
   }
   int T = forced_tile;
-  if (T == 0) T = (max_track <= 256 && n <= (1LL << 20)) ? 256 : 512;
+  if (T == 0) T = 256;  // three consumer groups of the pipelined matvec per SM
   while (T < max_track) T *= 2;
-  if (T != 256 && T != 512 && T != 1024) {
-    *err = "tile size must be 256, 512 or 1024";
+  if (T != 128 && T != 256 && T != 512 && T != 1024) {
+    *err = "tile size must be 128, 256, 512 or 1024";
     return CASPAR_BA_EINVAL;
   }
 
@@ -102,6 +102,8 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
   out->obs_of_slot.assign(out->n_slots > 0 ? out->n_slots : 1, -1);
   out->cam.assign(out->n_slots > 0 ? out->n_slots : 1, -1);
   out->rank.assign(out->n_slots > 0 ? out->n_slots : 1, 0);
+  // rank | local point id << 8, for the pipelined matvec (tiles of <= 256 slots: both fit a byte)
+  out->rankpid.assign(T <= 256 && out->n_slots > 0 ? out->n_slots : 1, 0);
   out->run_begin.assign(num_tiles + 1, 0);
 
   // --- 3. in-tile sort by (camera, point-major position) and run tables -------------------------
@@ -109,6 +111,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
 #pragma omp parallel
   {
     std::vector<unsigned long long> keys;
+    std::vector<unsigned short> pid_of_r;
 #pragma omp for schedule(dynamic, 64)
     for (int t = 0; t < num_tiles; ++t) {
       int base = out->pt_ptr[tile_pt[t]];
@@ -117,6 +120,9 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
       for (int r = 0; r < cnt; ++r)  // r = position in point-major order
         keys[r] = ((unsigned long long)cam_idx[obs_by_pt[base + r]] << 16) | (unsigned)r;
       std::sort(keys.begin(), keys.end());
+      pid_of_r.resize(cnt);
+      for (int a = tile_pt[t]; a < tile_pt[t + 1]; ++a)
+        for (int r = out->pt_ptr[a] - base; r < out->pt_ptr[a + 1] - base; ++r) pid_of_r[r] = (unsigned short)(a - tile_pt[t]);
       long long s0 = (long long)t * T;
       int runs = 0, prev = -1;
       for (int s = 0; s < cnt; ++s) {
@@ -124,6 +130,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
         out->obs_of_slot[s0 + s] = obs_by_pt[base + r];
         out->cam[s0 + s] = c;
         out->rank[s0 + s] = (unsigned short)r;
+        if (T <= 256) out->rankpid[s0 + s] = (unsigned short)(r | (pid_of_r[r] << 8));
         if (c != prev) { runs++; prev = c; }
       }
       runs_per_tile[t] = runs;

@@ -138,17 +138,18 @@ def test_track_over_the_limit_is_rejected():
     assert e.value.code == -1
 
 
-@pytest.mark.parametrize("tile", [256, 512, 1024])
+@pytest.mark.parametrize("tile", [128, 256, 512, 1024])
 @pytest.mark.parametrize("pipeline", ["0", "1"])
 def test_every_tile_size_and_both_matvec_kernels(scene_cache, monkeypatch, tile, pipeline):
-    """CASPAR_BA_TILE / CASPAR_BA_PIPELINE are read at create: T in {256, 512, 1024}; the one-block-per-tile
-    Schur pass and the persistent TMA-pipelined one must both match the oracle."""
+    """CASPAR_BA_TILE / CASPAR_BA_PIPELINE are read at create: T in {128, 256, 512, 1024}; the one-block-per-tile
+    Schur pass and the persistent TMA-pipelined one (tiles of <= 256 slots) must both match the oracle."""
     monkeypatch.setenv("CASPAR_BA_TILE", str(tile))
     monkeypatch.setenv("CASPAR_BA_PIPELINE", pipeline)
     s = scene_cache("mid", grid=(10, 12), num_points=40_000)
     g = pkg.CasparBA.from_scene(s)
     o = oracle.OracleBA.from_scene(s)
     assert g.stats().tile_slots == tile
+    assert g.stats().matvec_pipelined == (1 if pipeline == "1" and tile <= 256 else 0)
     _step_matches(g, o)
     p = np.random.default_rng(3).normal(size=9 * g.nc).astype(np.float32).astype(np.float64)
     assert rel_l2(g.schur_matvec(LAM, p), o.schur_matvec(LAM, p)) <= 1e-4
