@@ -86,6 +86,7 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.obs_of_slot = c.take<int>(S);
   v.rank = c.take<unsigned short>(S);
   v.rankpid = c.take<unsigned short>(ro.rankpid.size());
+  v.rankpid32 = c.take<unsigned>(ro.rankpid32.size());
   v.tile_pt = c.take<int>(ro.tile_pt.size());
   v.run_begin = c.take<int>(ro.run_begin.size());
   v.run_cam = c.take<int>(ro.run_cam.size());
@@ -185,6 +186,13 @@ int sync_step_scalars(caspar_ba* h, cudaStream_t s) {
   CK(cudaMemcpyAsync(h->h_pcg, h->v.pcg, sizeof(PcgScalars), cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
   if (h->profiling) drain_events(h);
+  double c = 0.0, tc = 0.0;
+  for (int i = 0; i < kCostSlots; ++i) {
+    c += h->h_step->cost_part[i];
+    tc += h->h_step->trial_part[i];
+  }
+  h->h_step->cost = c;
+  h->h_step->trial_cost = tc;
   return 0;
 }
 
@@ -337,7 +345,6 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
     const char* env = std::getenv("CASPAR_BA_PIPELINE");  // "0" selects the one-block-per-tile Schur pass
     v.pipeline = (!(env && env[0] == '0') && pipelined_matvec_possible(v)) ? 1 : 0;
   }
-  if (const char* env = std::getenv("CASPAR_BA_DEBUG")) v.dbg = std::atoi(env);
   h->camera_runs = ro.camera_runs;
   h->arena_bytes = carve(h, nullptr, ro);
   cudaError_t e = cudaMalloc(&h->arena, h->arena_bytes);
@@ -348,6 +355,7 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   if (e == cudaSuccess) e = upload(v.obs_of_slot, ro.obs_of_slot, s);
   if (e == cudaSuccess) e = upload(v.rank, ro.rank, s);
   if (e == cudaSuccess) e = upload(v.rankpid, ro.rankpid, s);
+  if (e == cudaSuccess) e = upload(v.rankpid32, ro.rankpid32, s);
   if (e == cudaSuccess) e = upload(v.tile_pt, ro.tile_pt, s);
   if (e == cudaSuccess) e = upload(v.run_begin, ro.run_begin, s);
   if (e == cudaSuccess) e = upload(v.run_cam, ro.run_cam, s);
@@ -423,10 +431,10 @@ int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
   cudaStream_t s = (cudaStream_t)cuda_stream;
   View& v = h->v;
   // evaluated in the trial buffers so that a cached linearization stays untouched
-  CK(cudaMemsetAsync(&v.step->trial_cost, 0, sizeof(double), s));
+  CK(cudaMemsetAsync(v.step->trial_part, 0, sizeof(double) * kCostSlots, s));
   CK(launch_pack_points(v, v.points, v.pts_trial, s));
   CK(launch_camera_prepass(v, v.cameras, v.cam_table_trial, s));
-  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
+  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, v.step->trial_part, s));
   account(h);
   int rc = sync_step_scalars(h, s);
   if (rc) return rc;
@@ -463,10 +471,10 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   rc = do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
   if (rc) return rc;
   // trial point and its cost (S9)
-  CK(cudaMemsetAsync(&v.step->trial_cost, 0, sizeof(double), s));
+  CK(cudaMemsetAsync(v.step->trial_part, 0, sizeof(double) * kCostSlots, s));
   CK(launch_trial_update(v, s));
   CK(launch_camera_prepass(v, v.cams_trial, v.cam_table_trial, s));
-  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
+  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, v.step->trial_part, s));
   account(h);
   rc = sync_step_scalars(h, s);  // the one host synchronisation of the step
   if (rc) return rc;

@@ -54,7 +54,12 @@ struct StepScalars {
   double dg;          // delta.g
   int bad_block;      // a 9x9 / 3x3 block was not positive definite
   int pad;
+  // the cost kernels add each warp's sum to one of kCostSlots slots (one address would serialise ~1e6 REDs
+  // in L2); the host folds the slots into cost / trial_cost after the copy
+  double cost_part[256];
+  double trial_part[256];
 };
+constexpr int kCostSlots = 256;
 
 // Everything the kernels need, passed by value.
 struct View {
@@ -72,7 +77,8 @@ struct View {
   const float2* px;
   const int* cam;
   const unsigned short* rank;
-  const unsigned short* rankpid;  // rank | local point id << 8 (T <= 256), read by the pipelined matvec
+  const unsigned short* rankpid;  // rank | local point id << 8 (T <= 256): linearize, pipelined matvec
+  const unsigned* rankpid32;      // rank | local point id << 16 (T > 256): linearize
   const int* obs_of_slot;  // caller observation id of a slot (-1 = padding)
   float4* J[6];
   float2* res;
@@ -90,7 +96,6 @@ struct View {
   const unsigned char* tile_meta;  // blobs
   int max_pts_per_tile, meta_max_bytes;
   int num_sms;
-  int dbg;                         // experiment knobs (CASPAR_BA_DEBUG), 0 in production
   int pipeline;                    // 1: Schur matvec runs as the persistent TMA-pipelined kernel
   // per internal point
   const int* pt_ptr;      // [np_obs + 1] prefix sum of track lengths
@@ -132,6 +137,7 @@ struct Reordered {
   std::vector<int> cam;                   // [n_slots]
   std::vector<unsigned short> rank;       // [n_slots]
   std::vector<unsigned short> rankpid;    // [n_slots] rank | local point id << 8 (tiles of <= 256 slots only)
+  std::vector<unsigned> rankpid32;        // [n_slots] rank | local point id << 16 (tiles of > 256 slots only)
   std::vector<int> tile_pt;               // [num_tiles + 1]
   std::vector<int> run_begin;             // [num_tiles + 1]
   std::vector<int> run_cam;

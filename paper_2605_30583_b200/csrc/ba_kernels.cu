@@ -229,29 +229,52 @@ constexpr int blocks_per_sm(int T) { return T == 128 ? 6 : (T == 256 ? 3 : (T ==
 // S2 + S3 (JAC = true): linearize every observation, store r and J, assemble V_k and g_p,k per point,
 //                       accumulate the cost.
 // S9      (JAC = false): residual-only cost at the given points / camera table.
+// One block per tile, one thread per observation.  The observation finds its point through the slot's
+// local point id (X_k is a 16-byte read from the tile's contiguous, L1-resident point range), so the only
+// block-wide step is the point-side reduction: the nine products V (6) and g_p (3) are scattered to the
+// point-major staging rows, and after ONE barrier lane (point, component) sums its range: three points
+// per warp and pass.
 // ------------------------------------------------------------------------------------------------
-template <int T, bool JAC>
-__global__ void __launch_bounds__(T, blocks_per_sm(T))
-linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict__ table, double* cost_acc) {
-  __shared__ float stage[JAC ? 9 : 3][T + 1];
-  __shared__ double red[32];
-  const int t = blockIdx.x, tid = threadIdx.x;
-  const long long slot = (long long)t * T + tid;
-  const int p0 = v.tile_pt[t], p1 = v.tile_pt[t + 1];
-  const int base = v.pt_ptr[p0];
-  const int cam = v.cam[slot];
-  const unsigned rank = v.rank[slot];
-  const float2 m = v.px[slot];
+template <int T>
+__device__ __forceinline__ void slot_rank_pid(const View& v, long long slot, unsigned& rank, unsigned& pid) {
+  if (T <= 256) {
+    const unsigned rp = v.rankpid[slot];
+    rank = rp & 255u;
+    pid = rp >> 8;
+  } else {
+    const unsigned rp = v.rankpid32[slot];
+    rank = rp & 0xffffu;
+    pid = rp >> 16;
+  }
+}
 
-  // point threads: scatter X_k to the point's range of ranks
-  for (int k = p0 + tid; k < p1; k += T) {
-    const float4 X = pts[k];
-    const int e = v.pt_ptr[k + 1] - base;
-    for (int r = v.pt_ptr[k] - base; r < e; ++r) {
-      stage[0][r] = X.x; stage[1][r] = X.y; stage[2][r] = X.z;
+template <int T, bool JAC>
+__global__ void __launch_bounds__(T, 1024 / T)
+linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict__ table, double* cost_acc) {
+  __shared__ float4 stage[JAC ? T : 1][2];  // by rank: (Vxx Vxy Vxz Vyy) (Vyz Vzz gx gy)
+  __shared__ float stage_gz[JAC ? T : 1];   // by rank: gz
+  __shared__ int arrived[JAC ? T : 1];      // by local point id: observations staged so far
+  const int t = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+  const long long slot = (long long)t * T + tid;
+  const int p0 = v.tile_pt[t];
+  const int cam = v.cam[slot];
+  unsigned rank, pid;
+  slot_rank_pid<T>(v, slot, rank, pid);
+  const float2 m = v.px[slot];
+  float4 X = make_float4(0.f, 0.f, 0.f, 0.f);
+  int rb = 0, re = 0;  // rank range of this observation's point
+  if (cam >= 0) {
+    X = __ldg(pts + p0 + pid);
+    if (JAC) {
+      const int base = __ldg(v.pt_ptr + p0);
+      rb = __ldg(v.pt_ptr + p0 + pid) - base;
+      re = __ldg(v.pt_ptr + p0 + pid + 1) - base;
     }
   }
-  __syncthreads();
+  if (JAC) {
+    arrived[tid] = 0;
+    __syncthreads();  // the only block-wide barrier: at the start, before anything has latency to expose
+  }
 
   float term = 0.f;
   if (JAC) {
@@ -259,7 +282,7 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
 #pragma unroll
     for (int i = 0; i < 24; ++i) J[i] = 0.f;
     if (cam >= 0) {
-      linearize_observation(table, cam, stage[0][rank], stage[1][rank], stage[2][rank], m, J, r0, r1);
+      linearize_observation(table, cam, X.x, X.y, X.z, m, J, r0, r1);
       const float s2 = fmaf(r0, r0, r1 * r1);
       if (v.robust) {  // Cauchy: w = 1 / (1 + s/c^2), r~ = sqrt(w) r, J~ = sqrt(w) J
         const float q = s2 / v.robust_c2;
@@ -272,46 +295,46 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
         term = s2;
       }
     }
-    // eager stores: six 128-bit chunk arrays + the residual
+    // eager stores: six 128-bit chunk arrays + the residual, streamed past L2's keep set
 #pragma unroll
-    for (int c = 0; c < 6; ++c) v.J[c][slot] = make_float4(J[4 * c], J[4 * c + 1], J[4 * c + 2], J[4 * c + 3]);
-    v.res[slot] = make_float2(r0, r1);
-    __syncthreads();  // every thread has read its X
+    for (int c = 0; c < 6; ++c) __stcs(&v.J[c][slot], make_float4(J[4 * c], J[4 * c + 1], J[4 * c + 2], J[4 * c + 3]));
+    __stcs(&v.res[slot], make_float2(r0, r1));
+    // Point side without a barrier: every observation stages its nine products at its rank, then counts
+    // itself in; the observation that completes its point sums the point's rank range IN RANK ORDER (so
+    // V_k and g_p,k do not depend on the arrival order) and writes the point's blocks.
     if (cam >= 0) {
-      stage[0][rank] = fmaf(J[18], J[18], J[21] * J[21]);
-      stage[1][rank] = fmaf(J[18], J[19], J[21] * J[22]);
-      stage[2][rank] = fmaf(J[18], J[20], J[21] * J[23]);
-      stage[3][rank] = fmaf(J[19], J[19], J[22] * J[22]);
-      stage[4][rank] = fmaf(J[19], J[20], J[22] * J[23]);
-      stage[5][rank] = fmaf(J[20], J[20], J[23] * J[23]);
-      stage[6][rank] = fmaf(J[18], r0, J[21] * r1);
-      stage[7][rank] = fmaf(J[19], r0, J[22] * r1);
-      stage[8][rank] = fmaf(J[20], r0, J[23] * r1);
-    }
-    __syncthreads();
-    for (int k = p0 + tid; k < p1; k += T) {
-      float acc[9];
-#pragma unroll
-      for (int c = 0; c < 9; ++c) acc[c] = 0.f;
-      const int e = v.pt_ptr[k + 1] - base;
-      for (int r = v.pt_ptr[k] - base; r < e; ++r) {
-#pragma unroll
-        for (int c = 0; c < 9; ++c) acc[c] += stage[c][r];
+      stage[rank][0] = make_float4(fmaf(J[18], J[18], J[21] * J[21]), fmaf(J[18], J[19], J[21] * J[22]),
+                                   fmaf(J[18], J[20], J[21] * J[23]), fmaf(J[19], J[19], J[22] * J[22]));
+      stage[rank][1] = make_float4(fmaf(J[19], J[20], J[22] * J[23]), fmaf(J[20], J[20], J[23] * J[23]),
+                                   fmaf(J[18], r0, J[21] * r1), fmaf(J[19], r0, J[22] * r1));
+      stage_gz[rank] = fmaf(J[20], r0, J[23] * r1);
+      __threadfence_block();
+      if (atomicAdd(&arrived[pid], 1) == re - rb - 1) {
+        __threadfence_block();
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+        float gz = 0.f;
+        for (int r = rb; r < re; ++r) {
+          const float4 x = stage[r][0], y = stage[r][1];
+          const float z = stage_gz[r];
+          a.x += x.x; a.y += x.y; a.z += x.z; a.w += x.w;
+          b.x += y.x; b.y += y.y; b.z += y.z; b.w += y.w;
+          gz += z;
+        }
+        v.V0[p0 + pid] = a;
+        v.V1[p0 + pid] = make_float2(b.x, b.y);
+        v.gp[p0 + pid] = make_float4(b.z, b.w, gz, 0.f);
       }
-      v.V0[k] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-      v.V1[k] = make_float2(acc[4], acc[5]);
-      v.gp[k] = make_float4(acc[6], acc[7], acc[8], 0.f);
     }
   } else {
     if (cam >= 0) {
       float r0, r1;
-      residual_observation(table, cam, stage[0][rank], stage[1][rank], stage[2][rank], m, r0, r1);
+      residual_observation(table, cam, X.x, X.y, X.z, m, r0, r1);
       const float s2 = fmaf(r0, r0, r1 * r1);
       term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
     }
   }
-  const double total = block_sum((double)term, red);
-  if (tid == 0) atomicAdd(cost_acc, total);
+  const double wsum = warp_sum((double)term);
+  if (lane == 0) atomicAdd(cost_acc + ((t * (T / 32) + (tid >> 5)) & (kCostSlots - 1)), wsum);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -830,7 +853,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       for (int k = 0; k < 9; ++k) rows[k * 33 + lane] = c9[k];
       camrow[lane] = cam;
       __syncwarp();
-      if (lane < 27 && !(v.dbg & 1)) {
+      if (lane < 27) {
         const int part = lane / 9, k = lane - 9 * part, s0 = 11 * part;
         const float* src = rows + k * 33 + s0;
         // bit i: slot s0 + i is the last slot of a segment (the next slot starts one), or of this part
@@ -1177,7 +1200,7 @@ static cudaError_t launch_linearize_t(const View& v, const float4* pts, const fl
 }
 
 cudaError_t launch_linearize(const View& v, cudaStream_t s) {
-  return launch_linearize_t<true>(v, v.pts, v.cam_table, &v.step->cost, s);
+  return launch_linearize_t<true>(v, v.pts, v.cam_table, v.step->cost_part, s);
 }
 
 cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_acc, cudaStream_t s) {

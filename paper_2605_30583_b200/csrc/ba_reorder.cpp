@@ -104,6 +104,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
   out->rank.assign(out->n_slots > 0 ? out->n_slots : 1, 0);
   // rank | local point id << 8, for the pipelined matvec (tiles of <= 256 slots: both fit a byte)
   out->rankpid.assign(T <= 256 && out->n_slots > 0 ? out->n_slots : 1, 0);
+  out->rankpid32.assign(T > 256 && out->n_slots > 0 ? out->n_slots : 1, 0);
   out->run_begin.assign(num_tiles + 1, 0);
 
   // --- 3. in-tile sort by (camera, point-major position) and run tables -------------------------
@@ -131,6 +132,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
         out->cam[s0 + s] = c;
         out->rank[s0 + s] = (unsigned short)r;
         if (T <= 256) out->rankpid[s0 + s] = (unsigned short)(r | (pid_of_r[r] << 8));
+        else out->rankpid32[s0 + s] = (unsigned)r | ((unsigned)pid_of_r[r] << 16);
         if (c != prev) { runs++; prev = c; }
       }
       runs_per_tile[t] = runs;
