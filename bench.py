@@ -166,6 +166,31 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------------
+# N > 1: the path does not shard ("replicas only"): every rank runs an independent replica of the
+# config on its own seed, there is no data-path collective; the only exchange is the timing reduction below
+# ---------------------------------------------------------------------------------------------------
+def replica_seed(config_seed: int, rank: int) -> int:
+    return config_seed + 1000 * rank
+
+
+def max_over_ranks(value: float, device=None) -> float:
+    """MAX of a per-rank scalar over the process group (identity without one)."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world: int, units_per_rank: float, ms_max: float) -> float:
+    """Units all ranks processed / the slowest rank's time (weak scaling: per-rank work is fixed)."""
+    return world * units_per_rank / (ms_max * 1e-3)
+
+
+# ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -189,7 +214,7 @@ def run_ours(args):
     kw = {}
     if args.shrink:                                   # debugging only; the bench line says so
         kw = SAMPLES[args.workload]
-    scene = make_scene(args.workload, seed=cfg["seed"] + 1000 * rank, **kw)
+    scene = make_scene(args.workload, seed=replica_seed(cfg["seed"], rank), **kw)
     n_obs = scene.num_observations
     cams0 = torch.from_numpy(scene.cameras).to(dev)
     pts0 = torch.from_numpy(scene.points).to(dev)
@@ -239,10 +264,7 @@ def run_ours(args):
     ms = start.elapsed_time(stop)
     st = gpu.stats()
     gpu.set_profiling(False)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+    ms_max = max_over_ranks(ms, dev)
     matvecs = sum(s.pcg_iterations for s in steps)
     lin_count = int(st.linearize_count)
 
@@ -257,10 +279,7 @@ def run_ours(args):
         run_steps(args.steps, (cam_h, pts_h))
         barrier()
         e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dev)
     param_bytes = 4 * (9 * scene.num_cameras + 3 * scene.num_points)
 
     if rank != 0:
@@ -283,7 +302,7 @@ def run_ours(args):
     mv_gbs = mv_bytes / (mv_ms * 1e-3) / 1e9 if mv_ms > 0 else 0.0
     lin_gbs = lin_bytes / (lin_ms * 1e-3) / 1e9 if lin_ms > 0 else 0.0
 
-    value = world * args.steps / (ms_max * 1e-3)
+    value = whole_job_rate(world, args.steps, ms_max)
     line = {
         "metric": "lm_iterations_per_s", "value": value, "unit": "LM iterations/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -293,7 +312,7 @@ def run_ours(args):
                    "pcg_max_iter": cap, "pcg_rel_tol": tol, "lambda0": LAMBDA0, "tile_slots": int(st.tile_slots),
                    "l2": "inputs larger than L2 (stored Jacobians %.2f GB per pass)" % (96.0 * n_obs / 1e9),
                    "replicas": world, "parallelism": "independent replicas, no collective"},
-        "schur_matvecs_per_s": world * matvecs / (ms_max * 1e-3), "matvecs_in_timed_region": matvecs,
+        "schur_matvecs_per_s": whole_job_rate(world, matvecs, ms_max), "matvecs_in_timed_region": matvecs,
         "linearizations_per_s": n_obs / (lin_ms * 1e-3) if lin_ms > 0 else None,
         "lm_costs": [s.cost_after for s in steps], "lm_accepted": [bool(s.accepted) for s in steps],
         "pcg_iterations": [s.pcg_iterations for s in steps],

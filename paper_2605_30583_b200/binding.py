@@ -262,11 +262,18 @@ class CasparBA:
         nc, np_, n = self.nc, self.np_, self.n
         shape = {RESIDUALS: (n, 2), JC: (n, 2, 9), JP: (n, 2, 3), U: (nc, 9, 9), V: (np_, 3, 3),
                  G: (9 * nc + 3 * np_,), SCHUR_RHS: (9 * nc,), DELTA: (9 * nc + 3 * np_,)}[what]
+        return self.export_device(what, stream).cpu().numpy()
+
+    def export_device(self, what: int, stream=None) -> torch.Tensor:
+        """The same export left on the device (fp64, caller's order): full-size tests sample it there."""
+        nc, np_, n = self.nc, self.np_, self.n
+        shape = {RESIDUALS: (n, 2), JC: (n, 2, 9), JP: (n, 2, 3), U: (nc, 9, 9), V: (np_, 3, 3),
+                 G: (9 * nc + 3 * np_,), SCHUR_RHS: (9 * nc,), DELTA: (9 * nc + 3 * np_,)}[what]
         count = int(np.prod(shape))
         out = torch.zeros(max(count, 1), dtype=torch.float64, device=self.device)
         self._check(self._lib.caspar_ba_export(self._h, what, out.data_ptr(), count, _stream_ptr(stream)),
                     f"export({what})")
-        return out[:count].cpu().numpy().reshape(shape)
+        return out[:count].reshape(shape)
 
     def schur_matvec(self, lam: float, p, stream=None) -> np.ndarray:
         p_dev = torch.as_tensor(np.asarray(p, dtype=np.float64)).to(self.device).contiguous()

@@ -689,10 +689,16 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   const int tid = threadIdx.x;
   unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L.bars);
   unsigned long long* empty = full + kMaxStages;
+  // seen[s]: how many fills of stage s some consumer has already observed complete.  A parity wait cannot tell
+  // "fill n done" from "fill n - 2 done, n - 1 still in flight"; when the stage count is not a multiple of NG
+  // the previous fill of a stage belongs to ANOTHER group, bulk copies may complete out of order, and a group
+  // could run one whole phase ahead of the barrier.  It therefore first waits until fill n - 1 has been seen.
+  volatile int* seen = reinterpret_cast<volatile int*>(empty + kMaxStages);
   if (tid == 0) {
     for (int s = 0; s < L.stages; ++s) {
       mbar_init(full + s, 1);
       mbar_init(empty + s, T / 32);  // one group consumes a stage
+      seen[s] = 0;
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     if (blockIdx.x == 0) {  // accumulators of the update that follows this matvec
@@ -748,9 +754,12 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   // diverge at lambda ~ 1e-5: DESIGN.md "PCG at tiny lambda").  fp64 accumulation.
   double dot_part = 0.0;
   int s = g % L.stages;  // stage of this group's current tile
-  unsigned ph = (unsigned)((g / L.stages) & 1);
+  int round = g / L.stages;  // which fill of that stage it is
   for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G) {
-    mbar_wait(full + s, ph);
+    while (seen[s] < round) {
+    }
+    mbar_wait(full + s, (unsigned)(round & 1));
+    if (gt == 0) seen[s] = round + 1;
     const unsigned char* st = smem + (size_t)s * L.stage_bytes;
     const int npts = reinterpret_cast<const int*>(st + L.meta)[0];
     const unsigned short* pt_start = reinterpret_cast<const unsigned short*>(st + L.meta + 16);
@@ -826,7 +835,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         const float s0 = sbuf[0][pid], s1 = sbuf[1][pid], s2 = sbuf[2][pid];
         e0 = u0 - fmaf(Jp[0], s0, fmaf(Jp[1], s1, Jp[2] * s2));
         e1 = u1 - fmaf(Jp[3], s0, fmaf(Jp[4], s1, Jp[5] * s2));
-        dot_part += (double)u0 * (double)e0 + (double)u1 * (double)e1;
+        dot_part += (double)fmaf(u0, e0, u1 * e1);  // O(1) magnitudes (the direction is normalised): no underflow
       }
       float J[20];  // J_c again, from the stage (cheaper than 18 registers held across two barriers)
 #pragma unroll
@@ -877,7 +886,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       __syncwarp();  // the scratch rows are rewritten by this warp's next tile
     }
     s += NG;
-    while (s >= L.stages) { s -= L.stages; ph ^= 1; }
+    while (s >= L.stages) { s -= L.stages; ++round; }
   }
   // p.q: one fp64 atomic per warp
   const double tot = warp_sum(dot_part);

@@ -2,10 +2,10 @@
 element by element on the same seeded scenes.  Tolerances are BASELINE.json north_star's, read as
 DESIGN.md C12 / C13 say:
 
-  residuals, Jacobians : |gpu - oracle| <= 1e-6 + 1e-5 * max(|oracle|, scale) per entry, scale = |uv| of the
-                         observation for residuals (fp32 cannot resolve the cancellation uv - pixel below
-                         ulp(uv)) and the largest entry of that observation's Jacobian row for Jacobians;
-                         and <= 1e-5 relative in L2 per array
+  residuals            : |gpu - oracle| <= 1e-6 + 1e-5 * |oracle| per entry (the literal reading; the GPU evaluates
+                         the projection in fp64) and <= 1e-5 relative in L2
+  Jacobians            : |gpu - oracle| <= 1e-6 + 1e-5 * max(|oracle|, largest entry of that observation's
+                         Jacobian row) per entry, and <= 1e-5 relative in L2 per array
   blocks U, V, gradient: <= 1e-5 (U, V) / 1e-4 (g, Schur rhs: signed sums that cancel) relative in L2
   Schur matvec, PCG step: <= 1e-4 relative in L2, both sides at the SAME iteration count (tol = 0)
   cost after the replayed LM schedule (the oracle's own (lambda_t, accepted_t) sequence): <= 1e-4 relative
@@ -64,9 +64,8 @@ def test_linearize_parity(pair, key):
     assert abs(cost_g - cost_o) <= 1e-5 * cost_o, (cost_g, cost_o)
 
     r_g, r_o = g.export(pkg.RESIDUALS), o.export(ob.RESIDUALS)
-    # |uv| of the observation bounds the fp32 rounding of the residual uv - pixel (C12)
-    scale = (np.abs(o.observations) + np.abs(r_o)).max(axis=1, keepdims=True)
-    assert (np.abs(r_g - r_o) <= 1e-6 + 1e-5 * scale).all(), float(np.max(np.abs(r_g - r_o) / scale))
+    # north_star's literal, entrywise reading: the GPU evaluates the projection in fp64 (C12)
+    assert (np.abs(r_g - r_o) <= 1e-6 + 1e-5 * np.abs(r_o)).all(), float(np.max(np.abs(r_g - r_o)))
     assert rel_l2(r_g, r_o) <= 1e-5
 
     for what_g, what_o in ((pkg.JC, ob.JC), (pkg.JP, ob.JP)):
