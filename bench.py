@@ -46,12 +46,16 @@ def hbm_peak():
 
 
 def ncu_traffic(kernel: str):
-    """dram bytes per launch of `kernel` from the committed ncu --set full summary, if any."""
+    """dram bytes per launch of `kernel` from the committed ncu --set full summary (profiles/r01_traffic.csv), if any."""
+    import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            return json.load(fh).get(kernel)
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
+            for row in csv.DictReader(fh):
+                if row["kernel"] == kernel:
+                    return float(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
