@@ -248,6 +248,16 @@ __device__ __forceinline__ void slot_rank_pid(const View& v, long long slot, uns
   }
 }
 
+// Thread `first + i` prefetches the i-th 128-byte line of [ptr, ptr + bytes) into L2; returns the next free thread.
+__device__ __forceinline__ int prefetch_lines(const void* ptr, long long bytes, int first, int tid) {
+  const char* p = reinterpret_cast<const char*>(ptr);
+  const char* line = reinterpret_cast<const char*>(reinterpret_cast<unsigned long long>(p) & ~127ull);
+  const int lines = (int)((p + bytes - line + 127) >> 7);
+  const int i = tid - first;
+  if (bytes > 0 && i >= 0 && i < lines) asm volatile("prefetch.global.L2 [%0];" ::"l"(line + 128ll * i));
+  return first + lines;
+}
+
 template <int T, bool JAC>
 __global__ void __launch_bounds__(T, 1024 / T)
 linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict__ table, double* cost_acc) {
@@ -261,6 +271,20 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
   unsigned rank, pid;
   slot_rank_pid<T>(v, slot, rank, pid);
   const float2 m = v.px[slot];
+  // Every block's critical path starts with two dependent levels of DRAM latency (slot arrays, then the point
+  // and rank-range gathers they address).  The block therefore pulls the inputs of the tile that will run one
+  // resident wave later (1024 / T blocks per SM) into L2: slot arrays now, points below.
+  const int tn = t + (1024 / T) * v.num_sms;
+  int np0 = 0, np1 = 0, next_thread = 0;
+  if (tn < v.num_tiles) {
+    np0 = __ldg(v.tile_pt + tn);
+    np1 = __ldg(v.tile_pt + tn + 1);
+    const long long sn = (long long)tn * T;
+    next_thread = prefetch_lines(v.cam + sn, T * 4, 0, tid);
+    next_thread = prefetch_lines(v.px + sn, T * 8, next_thread, tid);
+    next_thread = T <= 256 ? prefetch_lines(v.rankpid + sn, T * 2, next_thread, tid)
+                           : prefetch_lines(v.rankpid32 + sn, T * 4, next_thread, tid);
+  }
   float4 X = make_float4(0.f, 0.f, 0.f, 0.f);
   int rb = 0, re = 0;  // rank range of this observation's point
   if (cam >= 0) {
@@ -332,6 +356,10 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
       const float s2 = fmaf(r0, r0, r1 * r1);
       term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
     }
+  }
+  if (tn < v.num_tiles) {  // the next wave's points and rank ranges (their tile bounds have long arrived)
+    next_thread = prefetch_lines(pts + np0, 16ll * (np1 - np0), next_thread & (T - 1), tid);
+    if (JAC) prefetch_lines(v.pt_ptr + np0, 4ll * (np1 - np0 + 1), next_thread & (T - 1), tid);
   }
   const double wsum = warp_sum((double)term);
   if (lane == 0) atomicAdd(cost_acc + ((t * (T / 32) + (tid >> 5)) & (kCostSlots - 1)), wsum);
