@@ -335,18 +335,20 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
       __threadfence_block();
       if (atomicAdd(&arrived[pid], 1) == re - rb - 1) {
         __threadfence_block();
-        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+        float2 a0 = make_float2(0.f, 0.f), a1 = a0, b0 = a0, b1 = a0;
         float gz = 0.f;
-        for (int r = rb; r < re; ++r) {
+        for (int r = rb; r < re; ++r) {  // packed fp32 adds (FADD2)
           const float4 x = stage[r][0], y = stage[r][1];
           const float z = stage_gz[r];
-          a.x += x.x; a.y += x.y; a.z += x.z; a.w += x.w;
-          b.x += y.x; b.y += y.y; b.z += y.z; b.w += y.w;
+          a0 = __fadd2_rn(a0, make_float2(x.x, x.y));
+          a1 = __fadd2_rn(a1, make_float2(x.z, x.w));
+          b0 = __fadd2_rn(b0, make_float2(y.x, y.y));
+          b1 = __fadd2_rn(b1, make_float2(y.z, y.w));
           gz += z;
         }
-        v.V0[p0 + pid] = a;
-        v.V1[p0 + pid] = make_float2(b.x, b.y);
-        v.gp[p0 + pid] = make_float4(b.z, b.w, gz, 0.f);
+        v.V0[p0 + pid] = make_float4(a0.x, a0.y, a1.x, a1.y);
+        v.V1[p0 + pid] = b0;
+        v.gp[p0 + pid] = make_float4(b1.x, b1.y, gz, 0.f);
       }
     }
   } else {
