@@ -223,7 +223,7 @@ __device__ __forceinline__ void residual_observation(const float* __restrict__ t
   r1 = pr.r1;
 }
 
-constexpr int blocks_per_sm(int T) { return T == 128 ? 6 : (T == 256 ? 3 : (T == 512 ? 2 : 1)); }
+constexpr int blocks_per_sm(int T) { return T == 128 ? 6 : (T == 192 ? 4 : (T == 256 ? 3 : (T == 512 ? 2 : 1))); }
 
 // ------------------------------------------------------------------------------------------------
 // S2 + S3 (JAC = true): linearize every observation, store r and J, assemble V_k and g_p,k per point,
@@ -360,8 +360,8 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
     }
   }
   if (tn < v.num_tiles) {  // the next wave's points and rank ranges (their tile bounds have long arrived)
-    next_thread = prefetch_lines(pts + np0, 16ll * (np1 - np0), next_thread & (T - 1), tid);
-    if (JAC) prefetch_lines(v.pt_ptr + np0, 4ll * (np1 - np0 + 1), next_thread & (T - 1), tid);
+    next_thread = prefetch_lines(pts + np0, 16ll * (np1 - np0), next_thread % T, tid);
+    if (JAC) prefetch_lines(v.pt_ptr + np0, 4ll * (np1 - np0 + 1), next_thread % T, tid);
   }
   const double wsum = warp_sum((double)term);
   if (lane == 0) atomicAdd(cost_acc + ((t * (T / 32) + (tid >> 5)) & (kCostSlots - 1)), wsum);
@@ -1231,6 +1231,7 @@ static cudaError_t launch_linearize_t(const View& v, const float4* pts, const fl
   if (v.num_tiles == 0) return cudaSuccess;
   switch (v.T) {
     case 128: linearize_kernel<128, JAC><<<v.num_tiles, 128, 0, s>>>(v, pts, table, acc); break;
+    case 192: linearize_kernel<192, JAC><<<v.num_tiles, 192, 0, s>>>(v, pts, table, acc); break;
     case 256: linearize_kernel<256, JAC><<<v.num_tiles, 256, 0, s>>>(v, pts, table, acc); break;
     case 512: linearize_kernel<512, JAC><<<v.num_tiles, 512, 0, s>>>(v, pts, table, acc); break;
     default: linearize_kernel<1024, JAC><<<v.num_tiles, 1024, 0, s>>>(v, pts, table, acc); break;
@@ -1270,6 +1271,7 @@ static cudaError_t launch_pass(const View& v, int iter, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaSuccess;
   switch (v.T) {
     case 128: schur_pass_kernel<128, MODE><<<v.num_tiles, 128, 0, s>>>(v, iter); break;
+    case 192: schur_pass_kernel<192, MODE><<<v.num_tiles, 192, 0, s>>>(v, iter); break;
     case 256: schur_pass_kernel<256, MODE><<<v.num_tiles, 256, 0, s>>>(v, iter); break;
     case 512: schur_pass_kernel<512, MODE><<<v.num_tiles, 512, 0, s>>>(v, iter); break;
     default: schur_pass_kernel<1024, MODE><<<v.num_tiles, 1024, 0, s>>>(v, iter); break;
@@ -1294,7 +1296,7 @@ static int smem_optin() {
 
 // The pipelined matvec packs rank and local point id into 16 bits, so it serves tiles of <= 256 slots:
 // T = 256 with three consumer groups (800 threads) or T = 128 with six.  Longer tracks use schur_pass_kernel.
-static int pipe_groups(int T) { return T == 256 ? 3 : 6; }
+static int pipe_groups(int T) { return T == 256 ? 3 : (T == 192 ? 4 : 6); }
 
 bool pipelined_matvec_possible(const View& v) {
   if (v.num_tiles == 0 || v.T > 256) return false;
@@ -1313,6 +1315,8 @@ cudaError_t configure_kernels(const View& v) {
   if (!pipelined_matvec_available(v)) return cudaSuccess;
   if (v.T == 256)
     return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+  if (v.T == 192)
+    return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<192, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
   return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
 }
 
@@ -1322,6 +1326,8 @@ cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) {
   const int grid = v.num_tiles < v.num_sms ? v.num_tiles : v.num_sms;
   if (v.T == 256)
     schur_matvec_pipelined_kernel<256, 3><<<grid, 3 * 256 + 32, L.total, s>>>(v, iter, L);
+  else if (v.T == 192)
+    schur_matvec_pipelined_kernel<192, 4><<<grid, 4 * 192 + 32, L.total, s>>>(v, iter, L);
   else
     schur_matvec_pipelined_kernel<128, 6><<<grid, 6 * 128 + 32, L.total, s>>>(v, iter, L);
   return CBA_LAUNCHED();

@@ -46,9 +46,9 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
   }
   int T = forced_tile;
   if (T == 0) T = 256;  // three consumer groups of the pipelined matvec per SM
-  while (T < max_track) T *= 2;
-  if (T != 128 && T != 256 && T != 512 && T != 1024) {
-    *err = "tile size must be 128, 256, 512 or 1024";
+  while (T < max_track) T = T == 192 ? 256 : T * 2;
+  if (T != 128 && T != 192 && T != 256 && T != 512 && T != 1024) {
+    *err = "tile size must be 128, 192, 256, 512 or 1024";
     return CASPAR_BA_EINVAL;
   }
 

@@ -138,10 +138,10 @@ def test_track_over_the_limit_is_rejected():
     assert e.value.code == -1
 
 
-@pytest.mark.parametrize("tile", [128, 256, 512, 1024])
+@pytest.mark.parametrize("tile", [128, 192, 256, 512, 1024])
 @pytest.mark.parametrize("pipeline", ["0", "1"])
 def test_every_tile_size_and_both_matvec_kernels(scene_cache, monkeypatch, tile, pipeline):
-    """CASPAR_BA_TILE / CASPAR_BA_PIPELINE are read at create: T in {128, 256, 512, 1024}; the one-block-per-tile
+    """CASPAR_BA_TILE / CASPAR_BA_PIPELINE are read at create: T in {128, 192, 256, 512, 1024}; the one-block-per-tile
     Schur pass and the persistent TMA-pipelined one (tiles of <= 256 slots) must both match the oracle."""
     monkeypatch.setenv("CASPAR_BA_TILE", str(tile))
     monkeypatch.setenv("CASPAR_BA_PIPELINE", pipeline)
