@@ -321,11 +321,11 @@ def run_ours(args):
         "lm_costs": [s.cost_after for s in steps], "lm_accepted": [bool(s.accepted) for s in steps],
         "pcg_iterations": [s.pcg_iterations for s in steps],
         "roofline": {"kernel": "schur_matvec_pipelined_kernel<T>" if st.matvec_pipelined else "schur_pass_kernel<T,MATVEC>", "bound": "hbm", "achieved": mv_gbs, "peak": peak,
-                     "unit": "GB/s", "frac": mv_gbs / peak, "traffic": ncu_traffic("schur_matvec"),
+                     "unit": "GB/s", "frac": mv_gbs / peak, "traffic": ncu_traffic("schur_matvec") if args.workload == "large" and not args.shrink else None,
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": mv_bytes, "avg_launch_ms": mv_ms,
                      "launches_timed": int(matvecs), "launches_enqueued": int(st.matvec_count), "frac_of_nominal_8TBs": mv_gbs / 8000.0},
         "roofline_linearize": {"kernel": "linearize_kernel<T,true>", "bound": "hbm", "achieved": lin_gbs, "peak": peak,
-                               "unit": "GB/s", "frac": lin_gbs / peak, "traffic": ncu_traffic("linearize"),
+                               "unit": "GB/s", "frac": lin_gbs / peak, "traffic": ncu_traffic("linearize") if args.workload == "large" and not args.shrink else None,
                                "algorithmic_bytes_per_launch": lin_bytes, "avg_launch_ms": lin_ms,
                                "launches_timed": lin_count},
         "e2e": {"value": world * args.steps / e2e_s, "unit": "LM iterations/s", "h2d_bytes_per_step": param_bytes,
