@@ -275,8 +275,9 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
   // and rank-range gathers they address).  The block therefore pulls the inputs of the tile that will run one
   // resident wave later (1024 / T blocks per SM) into L2: slot arrays now, points below.
   const int tn = t + (1024 / T) * v.num_sms;
+  const bool prefetcher = tid < 64 && tn < v.num_tiles;  // two warps issue the (at most ~40) line prefetches
   int np0 = 0, np1 = 0, next_thread = 0;
-  if (tn < v.num_tiles) {
+  if (prefetcher) {
     np0 = __ldg(v.tile_pt + tn);
     np1 = __ldg(v.tile_pt + tn + 1);
     const long long sn = (long long)tn * T;
@@ -359,9 +360,9 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
       term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
     }
   }
-  if (tn < v.num_tiles) {  // the next wave's points and rank ranges (their tile bounds have long arrived)
-    next_thread = prefetch_lines(pts + np0, 16ll * (np1 - np0), next_thread % T, tid);
-    if (JAC) prefetch_lines(v.pt_ptr + np0, 4ll * (np1 - np0 + 1), next_thread % T, tid);
+  if (prefetcher) {  // the next wave's points and rank ranges (their tile bounds have long arrived)
+    next_thread = prefetch_lines(pts + np0, 16ll * (np1 - np0), next_thread % 64, tid);
+    if (JAC) prefetch_lines(v.pt_ptr + np0, 4ll * (np1 - np0 + 1), next_thread % 64, tid);
   }
   const double wsum = warp_sum((double)term);
   if (lane == 0) atomicAdd(cost_acc + ((t * (T / 32) + (tid >> 5)) & (kCostSlots - 1)), wsum);
