@@ -696,7 +696,7 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   L.vinv = up(L.rank + T * 2);
   L.meta = up(L.vinv + max_pts * 32);
   L.stage_bytes = up(L.meta + meta_max);
-  L.tbuf_bytes = up(3 * (T + 1) * 4);
+  L.tbuf_bytes = up(3 * (T + 2) * 4);
   L.sbuf_bytes = up(3 * (T + 1) * 4);
   const int fixed = NG * (L.tbuf_bytes + L.sbuf_bytes) + NG * (T / 32) * kWarpScratchBytes + 256;
   int st = (smem_limit - fixed) / L.stage_bytes;
@@ -776,7 +776,8 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   // ===== consumers: group g takes every NG-th tile of this CTA's sequence =====
   const int g = tid / T, gt = tid - g * T, lane = tid & 31;
   const int bar_id = 1 + g;
-  float(*tbuf)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.tbuf + (size_t)g * L.tbuf_bytes);  // by rank
+  // row stride T + 2: the six lanes of a point in phase B (component c, half h) read banks 2c + h + rank: distinct
+  float(*tbuf)[T + 2] = reinterpret_cast<float(*)[T + 2]>(smem + L.tbuf + (size_t)g * L.tbuf_bytes);  // by rank
   float(*sbuf)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // by point
   float* rows = reinterpret_cast<float*>(smem + L.scratch + (size_t)(tid >> 5) * kWarpScratchBytes);
   int* camrow = reinterpret_cast<int*>(rows + 9 * 33);
