@@ -40,7 +40,15 @@ struct caspar_ba {
   long long lin_n = 0, mv_n = 0;
   std::vector<cudaEvent_t> ev_pool;
   cudaEvent_t poll_ev[2] = {nullptr, nullptr};
+  // one chunk of PCG iterations (matvec + two update kernels, kPcgChunk times) as an instantiated CUDA graph:
+  // no kernel argument changes between iterations (the iteration number is a device scalar), so the same graph
+  // serves every chunk of every solve; captured once per handle on a private stream, launched on the caller's
+  cudaStream_t capture_stream = nullptr;
+  cudaGraphExec_t chunk_graph = nullptr;
+  bool graph_tried = false;
 };
+
+constexpr int kPcgChunk = 8;
 
 namespace {
 
@@ -223,6 +231,25 @@ int do_prepare(caspar_ba* h, double lambda, cudaStream_t s) {
   return 0;
 }
 
+// Capture one chunk of iterations.  Failure is not an error: the loop then launches the kernels one by one.
+static void build_chunk_graph(caspar_ba* h) {
+  h->graph_tried = true;
+  if (const char* env = std::getenv("CASPAR_BA_GRAPH"))
+    if (env[0] == '0') return;
+  if (cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking) != cudaSuccess) return;
+  cudaGraph_t graph = nullptr;
+  bool ok = cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  for (int i = 0; ok && i < kPcgChunk; ++i)
+    ok = launch_schur_matvec(h->v, h->capture_stream) == cudaSuccess &&
+         launch_pcg_update(h->v, h->capture_stream) == cudaSuccess;
+  const cudaError_t end = cudaStreamEndCapture(h->capture_stream, &graph);
+  take_launch_count();  // captured launches are counted when the graph is launched
+  if (ok && end == cudaSuccess && graph && cudaGraphInstantiate(&h->chunk_graph, graph, 0) != cudaSuccess)
+    h->chunk_graph = nullptr;
+  if (graph) cudaGraphDestroy(graph);
+  cudaGetLastError();
+}
+
 // Enqueue S5-S8.  No host synchronisation unless rel_tol > 0, where the device-side `done` flag is
 // polled one chunk behind the launches so that the GPU never waits for the host.
 int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream_t s) {
@@ -233,17 +260,29 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
   if (rc) return rc;
   CK(cudaMemsetAsync(v.pcg, 0, sizeof(PcgScalars), s));
   CK(launch_schur_rhs(v, s));
-  CK(launch_pcg_init(v, s));
   const double tol2 = rel_tol * rel_tol;
-  const int chunk = 8;
+  CK(launch_pcg_init(v, tol2, s));
+  const int chunk = kPcgChunk;
+  // whole chunks go out as one graph launch (not while per-launch profiling events are wanted)
+  if (!h->graph_tried && v.nc > 0 && v.num_tiles > 0) {
+    account(h);
+    build_chunk_graph(h);
+  }
+  const bool use_graph = h->chunk_graph != nullptr && !h->profiling;
   int polled = 0;  // chunks whose flag copy has been enqueued
   bool stop = false;
   for (int it = 0; it < max_iter && !stop; ++it) {
-    {
-      Timed t(h, &h->ev_mv, s);
-      CK(launch_schur_matvec(v, it, s));
+    if (use_graph && it % chunk == 0 && it + chunk <= max_iter) {
+      CK(cudaGraphLaunch(h->chunk_graph, s));
+      h->launches += 3ll * chunk;
+      it += chunk - 1;
+    } else {
+      {
+        Timed t(h, &h->ev_mv, s);
+        CK(launch_schur_matvec(v, s));
+      }
+      CK(launch_pcg_update(v, s));
     }
-    CK(launch_pcg_update(v, it, tol2, s));
     if (rel_tol > 0.0 && (it + 1) % chunk == 0 && it + 1 < max_iter) {
       const int slot = polled & 1;
       if (polled >= 2) {  // wait for the copy enqueued two chunks ago (slot reuse) and look at it
@@ -403,6 +442,8 @@ void caspar_ba_destroy(caspar_ba_t* h) {
   for (cudaEvent_t e : h->ev_mv) cudaEventDestroy(e);
   for (cudaEvent_t e : h->poll_ev)
     if (e) cudaEventDestroy(e);
+  if (h->chunk_graph) cudaGraphExecDestroy(h->chunk_graph);
+  if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
   if (h->h_pcg) cudaFreeHost(h->h_pcg);
   if (h->h_step) cudaFreeHost(h->h_step);
   if (h->h_flags) cudaFreeHost(h->h_flags);

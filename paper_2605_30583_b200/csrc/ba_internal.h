@@ -40,6 +40,9 @@ struct PcgScalars {
   double bnorm2;  // |b|^2
   double rz0;
   double pscale;  // the fp32 direction handed to the matvec is p * pscale (a power of two)
+  double tol2;    // squared relative tolerance of this solve
+  int it_a;       // iteration number: read by the matvec and pcg_update_xr, written by pcg_update_p
+  int it_b;       // the same, read by pcg_update_p, written by pcg_update_xr
   int done;       // set once converged / broken down: every later kernel returns immediately
   int converged;
   int breakdown;  // p.Sp <= 0 or non-finite
@@ -165,13 +168,13 @@ cudaError_t launch_cost(const View& v, const float4* pts, const float* table, do
 cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s);
 cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s);
 cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);
-cudaError_t launch_pcg_init(const View& v, cudaStream_t s);
-cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s);
+cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s);
+cudaError_t launch_schur_matvec(const View& v, cudaStream_t s);
 cudaError_t configure_kernels(const View& v);  // once per handle: dynamic shared memory opt-in
 bool pipelined_matvec_possible(const View& v);   // shape / shared-memory check, at create
 bool pipelined_matvec_available(const View& v);  // = v.pipeline
 int pipeline_stages(const View& v);
-cudaError_t launch_pcg_update(const View& v, int iter, double tol2, cudaStream_t s);  // two kernels
+cudaError_t launch_pcg_update(const View& v, cudaStream_t s);  // two kernels
 cudaError_t launch_backsub(const View& v, cudaStream_t s);
 cudaError_t launch_trial_update(const View& v, cudaStream_t s);
 cudaError_t launch_commit(const View& v, cudaStream_t s);

@@ -510,14 +510,14 @@ __global__ void prepare_points_kernel(View v, double lambda) {
 enum { MATVEC = 0, RHS = 1, BACKSUB = 2 };
 
 template <int T, int MODE>
-__global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v, int iter) {
+__global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v) {
   __shared__ float stage[9][T + 1];
   __shared__ double red[32];
   const int t = blockIdx.x, tid = threadIdx.x;
   if (MODE == MATVEC) {
     if (v.pcg->done) return;
     if (t == 0 && tid == 0) {  // accumulators of the update that follows this matvec
-      const int nxt = (iter + 1) & 1;
+      const int nxt = (v.pcg->it_a + 1) & 1;  // it_a: written by the previous update kernel only
       v.pcg->rz[nxt] = 0.0;
       v.pcg->pDp[nxt] = 0.0;
       v.pcg->rr = 0.0;
@@ -714,7 +714,7 @@ __device__ __forceinline__ void group_bar(int id, int threads) {
 }
 
 template <int T, int NG>
-__global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(View v, int iter, PipeLayout L) {
+__global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(View v, PipeLayout L) {
   extern __shared__ __align__(128) unsigned char smem[];
   if (v.pcg->done) return;
   const int tid = threadIdx.x;
@@ -733,7 +733,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     if (blockIdx.x == 0) {  // accumulators of the update that follows this matvec
-      const int nxt = (iter + 1) & 1;
+      const int nxt = (v.pcg->it_a + 1) & 1;  // it_a: written by the previous update kernel only
       v.pcg->rz[nxt] = 0.0;
       v.pcg->pDp[nxt] = 0.0;
       v.pcg->rr = 0.0;
@@ -958,7 +958,7 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_norm_kernel(View v) {
 }
 
 // x = 0, r = b, z = M^-1 r, p = z; rz[0], |r|^2, pDp[0]
-__global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v) {
+__global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v, double tol2) {
   __shared__ double rs[kPcgThreads];
   __shared__ double red[32];
   const int tid = threadIdx.x;
@@ -987,16 +987,23 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v) {
     atomicAdd(&v.pcg->rz[0], s_rz);
     atomicAdd(&v.pcg->rr, s_rr);
     atomicAdd(&v.pcg->pDp[0], s_pd);
-    if (blockIdx.x == 0) v.pcg->pscale = scale;
+    if (blockIdx.x == 0) {
+      v.pcg->pscale = scale;
+      v.pcg->tol2 = tol2;
+    }
   }
 }
 
 // alpha = rz / (p.q); x += alpha p; r -= alpha q; z = M^-1 r; rz_new, |r|^2
-__global__ void __launch_bounds__(kPcgThreads) pcg_update_xr_kernel(View v, int iter) {
+// The iteration number lives on the device (it_a: read by the matvec and by this kernel, written by
+// pcg_update_p; it_b: read by pcg_update_p, written here): no kernel reads a counter it writes, and no kernel
+// argument changes from one iteration to the next, so a chunk of iterations can be replayed as a CUDA graph.
+__global__ void __launch_bounds__(kPcgThreads) pcg_update_xr_kernel(View v) {
   __shared__ double rs[kPcgThreads];
   __shared__ double red[32];
   PcgScalars* sc = v.pcg;
   if (sc->done) return;
+  const int iter = sc->it_a;
   const int tid = threadIdx.x, par = iter & 1;
   const double unscale = 1.0 / sc->pscale;  // q and p.q were computed from p * pscale
   const double denom = sc->pq * unscale * unscale + sc->pDp[par];
@@ -1034,18 +1041,20 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_xr_kernel(View v, int 
     atomicAdd(&sc->rr, s_rr);
     if (blockIdx.x == 0) {
       sc->iters = iter + 1;
+      sc->it_b = iter;
       if (iter == 0) sc->rz0 = rz;
     }
   }
 }
 
 // stop if |r| <= tol |b|, else beta = rz_new / rz; p = z + beta p; p.(lambda D p); q = 0
-__global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v, int iter, double tol2) {
+__global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v) {
   __shared__ double red[32];
   PcgScalars* sc = v.pcg;
   if (sc->done) return;
+  const int iter = sc->it_b;
   const int tid = threadIdx.x, par = iter & 1;
-  if (sc->rr <= tol2 * sc->bnorm2) {
+  if (sc->rr <= sc->tol2 * sc->bnorm2) {
     if (blockIdx.x == 0 && tid == 0) { sc->done = 1; sc->converged = 1; }
     return;
   }
@@ -1067,6 +1076,7 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v, int i
     if (blockIdx.x == 0) {
       sc->pq = 0.0;
       sc->pscale = scale;
+      sc->it_a = iter + 1;
     }
   }
 }
@@ -1269,19 +1279,19 @@ cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s) 
 }
 
 template <int MODE>
-static cudaError_t launch_pass(const View& v, int iter, cudaStream_t s) {
+static cudaError_t launch_pass(const View& v, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaSuccess;
   switch (v.T) {
-    case 128: schur_pass_kernel<128, MODE><<<v.num_tiles, 128, 0, s>>>(v, iter); break;
-    case 192: schur_pass_kernel<192, MODE><<<v.num_tiles, 192, 0, s>>>(v, iter); break;
-    case 256: schur_pass_kernel<256, MODE><<<v.num_tiles, 256, 0, s>>>(v, iter); break;
-    case 512: schur_pass_kernel<512, MODE><<<v.num_tiles, 512, 0, s>>>(v, iter); break;
-    default: schur_pass_kernel<1024, MODE><<<v.num_tiles, 1024, 0, s>>>(v, iter); break;
+    case 128: schur_pass_kernel<128, MODE><<<v.num_tiles, 128, 0, s>>>(v); break;
+    case 192: schur_pass_kernel<192, MODE><<<v.num_tiles, 192, 0, s>>>(v); break;
+    case 256: schur_pass_kernel<256, MODE><<<v.num_tiles, 256, 0, s>>>(v); break;
+    case 512: schur_pass_kernel<512, MODE><<<v.num_tiles, 512, 0, s>>>(v); break;
+    default: schur_pass_kernel<1024, MODE><<<v.num_tiles, 1024, 0, s>>>(v); break;
   }
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pass<RHS>(v, 0, s); }
+cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pass<RHS>(v, s); }
 
 // The pipelined matvec needs the opt-in shared-memory limit and at least two stages; otherwise (or with
 // CASPAR_BA_PIPELINE=0) the one-block-per-tile kernel is used.
@@ -1322,35 +1332,35 @@ cudaError_t configure_kernels(const View& v) {
   return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
 }
 
-cudaError_t launch_schur_matvec(const View& v, int iter, cudaStream_t s) {
-  if (!pipelined_matvec_available(v)) return launch_pass<MATVEC>(v, iter, s);
+cudaError_t launch_schur_matvec(const View& v, cudaStream_t s) {
+  if (!pipelined_matvec_available(v)) return launch_pass<MATVEC>(v, s);
   const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
   const int grid = v.num_tiles < v.num_sms ? v.num_tiles : v.num_sms;
   if (v.T == 256)
-    schur_matvec_pipelined_kernel<256, 3><<<grid, 3 * 256 + 32, L.total, s>>>(v, iter, L);
+    schur_matvec_pipelined_kernel<256, 3><<<grid, 3 * 256 + 32, L.total, s>>>(v, L);
   else if (v.T == 192)
-    schur_matvec_pipelined_kernel<192, 4><<<grid, 4 * 192 + 32, L.total, s>>>(v, iter, L);
+    schur_matvec_pipelined_kernel<192, 4><<<grid, 4 * 192 + 32, L.total, s>>>(v, L);
   else
-    schur_matvec_pipelined_kernel<128, 6><<<grid, 6 * 128 + 32, L.total, s>>>(v, iter, L);
+    schur_matvec_pipelined_kernel<128, 6><<<grid, 6 * 128 + 32, L.total, s>>>(v, L);
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_pcg_init(const View& v, cudaStream_t s) {
+cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s) {
   if (v.nc == 0) return cudaSuccess;
   pcg_norm_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
   cudaError_t e = CBA_LAUNCHED();
   if (e != cudaSuccess) return e;
-  pcg_init_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
+  pcg_init_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v, tol2);
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_pcg_update(const View& v, int iter, double tol2, cudaStream_t s) {
+cudaError_t launch_pcg_update(const View& v, cudaStream_t s) {
   if (v.nc == 0) return cudaSuccess;
   const unsigned g = grid_for(9ll * v.nc, kPcgThreads);
-  pcg_update_xr_kernel<<<g, kPcgThreads, 0, s>>>(v, iter);
+  pcg_update_xr_kernel<<<g, kPcgThreads, 0, s>>>(v);
   cudaError_t e = CBA_LAUNCHED();
   if (e != cudaSuccess) return e;
-  pcg_update_p_kernel<<<g, kPcgThreads, 0, s>>>(v, iter, tol2);
+  pcg_update_p_kernel<<<g, kPcgThreads, 0, s>>>(v);
   return CBA_LAUNCHED();
 }
 
@@ -1361,7 +1371,7 @@ cudaError_t launch_backsub(const View& v, cudaStream_t s) {
     e = CBA_LAUNCHED();
   }
   if (e != cudaSuccess) return e;
-  return launch_pass<BACKSUB>(v, 0, s);
+  return launch_pass<BACKSUB>(v, s);
 }
 
 cudaError_t launch_trial_update(const View& v, cudaStream_t s) {
@@ -1399,7 +1409,7 @@ cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* 
   matvec_load_kernel<<<g, 256, 0, s>>>(v, p_in);
   cudaError_t e = CBA_LAUNCHED();
   if (e != cudaSuccess) return e;
-  e = launch_schur_matvec(v, 0, s);
+  e = launch_schur_matvec(v, s);
   if (e != cudaSuccess) return e;
   matvec_finish_kernel<<<g, 256, 0, s>>>(v, q_out);
   return CBA_LAUNCHED();

@@ -186,3 +186,20 @@ def test_host_parameter_round_trip(scene_cache):
     so = o.lm_step(LAM, 0.0, 20, accept_mode=1)
     assert abs(st.cost_after - so.cost_after) <= 1e-4 * so.cost_after
     g.close()
+
+
+@pytest.mark.parametrize("graph", ["0", "1"])
+def test_pcg_chunks_as_a_cuda_graph_and_kernel_by_kernel_agree(scene_cache, monkeypatch, graph):
+    """CASPAR_BA_GRAPH=0 launches every PCG kernel on its own; by default whole chunks of 8 iterations are one
+    CUDA-graph launch and the remainder (25 = 3 x 8 + 1) goes kernel by kernel.  Same iteration counts, same step;
+    the tolerance-driven run stops at the same place."""
+    monkeypatch.setenv("CASPAR_BA_GRAPH", graph)
+    s = scene_cache("small")
+    g = pkg.CasparBA.from_scene(s)
+    o = oracle.OracleBA.from_scene(s)
+    _step_matches(g, o, iters=25)
+    ig, io = g.pcg_solve(LAM, 1e-6, 100), o.pcg_solve(LAM, 1e-6, 100)
+    assert ig.converged and io.converged and abs(ig.iterations - io.iterations) <= 1
+    assert rel_l2(g.export(pkg.DELTA), o.export(ob.DELTA)) <= 1e-4
+    g.close()
+    o.close()
