@@ -106,6 +106,8 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.cslot = c.take<int>(ro.cslot.size());
   v.chunk_cam = c.take<int>(ro.chunk_cam.size());
   v.chunk_begin = c.take<int>(ro.chunk_begin.size());
+  v.hot_of_cam = c.take<short>(ro.hot_of_cam.size());
+  v.hot_list = c.take<int>(ro.hot_list.size());
   v.pts = c.take<float4>(NP);
   v.pts_trial = c.take<float4>(NP);
   v.V0 = c.take<float4>(NP);
@@ -367,6 +369,7 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   v.num_tiles = ro.num_tiles;
   v.n_slots = ro.n_slots;
   v.num_chunks = (int)ro.chunk_cam.size();
+  v.num_hot = (int)ro.hot_list.size();
   v.robust = pb->robust_loss;
   v.robust_c2 = pb->robust_scale * pb->robust_scale;
   v.damping_mode = pb->damping_mode;
@@ -406,6 +409,8 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   if (e == cudaSuccess) e = upload(v.cslot, ro.cslot, s);
   if (e == cudaSuccess) e = upload(v.chunk_cam, ro.chunk_cam, s);
   if (e == cudaSuccess) e = upload(v.chunk_begin, ro.chunk_begin, s);
+  if (e == cudaSuccess) e = upload(v.hot_of_cam, ro.hot_of_cam, s);
+  if (e == cudaSuccess) e = upload(v.hot_list, ro.hot_list, s);
   // pixels: the caller's array may live on either side; stage through the device if it is host memory
   float* obs_dev = nullptr;
   if (e == cudaSuccess && n > 0) {

@@ -29,6 +29,7 @@ constexpr int kCamTableFloats = 36;  // per-camera table row (9 x 16 B: 12 doubl
 constexpr int kCamPad = 12;          // fp32 camera-vector copies (p, delta_c) are padded 9 -> 12 floats
 constexpr int kUg = 54;              // 45 upper-triangle entries of U_j + 9 of g_c,j, fp64 accumulators
 constexpr int kChunkSlots = 1024;    // camera-ordered assembly: slots per work item
+constexpr int kMaxHotCameras = 128;  // cameras whose q rows the pipelined matvec accumulates per CTA
 constexpr float kDMin = 1e-6f;       // floor of diag(J^T J) in the damping matrix (C5)
 
 // Scalars of the PCG recurrence, device resident (no host round trip inside the loop).
@@ -128,6 +129,10 @@ struct View {
   const int* chunk_cam;   // [num_chunks]
   const int* chunk_begin; // [num_chunks + 1] into cslot
   const int* cslot;       // slots grouped by camera, ascending
+  // hot cameras (far more observations than average): index into the per-CTA accumulators, or -1
+  const short* hot_of_cam;  // [nc]
+  const int* hot_list;      // [num_hot] camera ids
+  int num_hot;
   PcgScalars* pcg;
   StepScalars* step;
 };
@@ -148,6 +153,8 @@ struct Reordered {
   std::vector<int> pt_ptr;                // [np_obs + 1]
   std::vector<int> pt_perm;               // [np]
   std::vector<int> chunk_cam, chunk_begin, cslot;
+  std::vector<short> hot_of_cam;          // [nc]
+  std::vector<int> hot_list;
   std::vector<int> tile_dir;              // [4 * num_tiles]
   std::vector<unsigned char> tile_meta;
   int max_pts_per_tile = 0, meta_max_bytes = 0;

@@ -678,7 +678,7 @@ __device__ __forceinline__ void consumer_bar() {
 
 struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
   int j, cam, rank, vinv, meta, stage_bytes;
-  int stages, groups, tbuf, tbuf_bytes, sbuf, sbuf_bytes, scratch, bars, total;
+  int stages, groups, tbuf, tbuf_bytes, sbuf, sbuf_bytes, scratch, hot, bars, total;
 };
 
 constexpr int kMaxStages = 12;
@@ -686,7 +686,8 @@ constexpr int kWarpScratchBytes = 1408;  // per consumer warp: 9 x 33 floats of 
 
 // NG consumer groups of T threads share the ring; each group owns a staging area for the point-side sums
 // t_k (by rank) and one for the per-point results s_k (by local point id).
-__host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, int meta_max, int smem_limit) {
+__host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, int meta_max, int num_hot,
+                                                  int smem_limit) {
   PipeLayout L;
   auto up = [](int x) { return (x + 127) & ~127; };
   L.groups = NG;
@@ -698,13 +699,15 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   L.stage_bytes = up(L.meta + meta_max);
   L.tbuf_bytes = up(3 * (T + 2) * 4);
   L.sbuf_bytes = up(3 * (T + 1) * 4);
-  const int fixed = NG * (L.tbuf_bytes + L.sbuf_bytes) + NG * (T / 32) * kWarpScratchBytes + 256;
+  const int hot_bytes = up(num_hot * 9 * 8);  // per-CTA fp64 accumulators of the hot cameras' q rows
+  const int fixed = NG * (L.tbuf_bytes + L.sbuf_bytes) + NG * (T / 32) * kWarpScratchBytes + hot_bytes + 256;
   int st = (smem_limit - fixed) / L.stage_bytes;
   L.stages = st > kMaxStages ? kMaxStages : st;
   L.tbuf = L.stages * L.stage_bytes;
   L.sbuf = L.tbuf + NG * L.tbuf_bytes;
   L.scratch = L.sbuf + NG * L.sbuf_bytes;
-  L.bars = L.scratch + NG * (T / 32) * kWarpScratchBytes;
+  L.hot = L.scratch + NG * (T / 32) * kWarpScratchBytes;
+  L.bars = L.hot + hot_bytes;
   L.total = L.bars + 256;
   return L;
 }
@@ -713,7 +716,7 @@ __device__ __forceinline__ void group_bar(int id, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
-template <int T, int NG>
+template <int T, int NG, bool HOT>
 __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(View v, PipeLayout L) {
   extern __shared__ __align__(128) unsigned char smem[];
   if (v.pcg->done) return;
@@ -725,6 +728,11 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   // the previous fill of a stage belongs to ANOTHER group, bulk copies may complete out of order, and a group
   // could run one whole phase ahead of the barrier.  It therefore first waits until fill n - 1 has been seen.
   volatile int* seen = reinterpret_cast<volatile int*>(empty + kMaxStages);
+  // Hot cameras (Zipf popularity: one camera can hold 16 % of the observations) would serialise ~1e5 REDs on the
+  // same three L2 sectors per matvec; their rows are accumulated here, per CTA, and added to q once at the end.
+  double* hot_acc = reinterpret_cast<double*>(smem + L.hot);
+  if (HOT)
+    for (int i = tid; i < 9 * v.num_hot; i += NG * T + 32) hot_acc[i] = 0.0;
   if (tid == 0) {
     for (int s = 0; s < L.stages; ++s) {
       mbar_init(full + s, 1);
@@ -910,7 +918,11 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
           acc += val[i];
           if (endm & (1u << i)) {
             const int cm = camrow[s0 + i];
-            if (cm >= 0) atomicAdd(qk + 9ll * cm, (double)acc);
+            if (cm >= 0) {
+              const int hot = HOT ? (int)__ldg(v.hot_of_cam + cm) : -1;
+              if (hot >= 0) atomicAdd(hot_acc + 9 * hot + k, (double)acc);
+              else atomicAdd(qk + 9ll * cm, (double)acc);
+            }
             acc = 0.f;
           }
         }
@@ -923,6 +935,13 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   // p.q: one fp64 atomic per warp
   const double tot = warp_sum(dot_part);
   if (lane == 0) atomicAdd(&v.pcg->pq, tot);
+  if (HOT) {  // all consumer groups are done: one RED per hot camera row and CTA
+    group_bar(15, NG * T);
+    for (int i = tid; i < 9 * v.num_hot; i += NG * T) {
+      const double a = hot_acc[i];
+      if (a != 0.0) atomicAdd(v.q + 9ll * __ldg(v.hot_list + i / 9) + i % 9, a);
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1312,36 +1331,46 @@ static int pipe_groups(int T) { return T == 256 ? 3 : (T == 192 ? 4 : 6); }
 
 bool pipelined_matvec_possible(const View& v) {
   if (v.num_tiles == 0 || v.T > 256) return false;
-  const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
+  const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, v.num_hot, smem_optin());
   return L.stages >= pipe_groups(v.T) + 1;
 }
 
 bool pipelined_matvec_available(const View& v) { return v.pipeline != 0; }
 int pipeline_stages(const View& v) {
-  return pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin()).stages;
+  return pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, v.num_hot, smem_optin()).stages;
 }
 
 // The opt-in limit itself is requested (not this handle's own size): the attribute is per function, and
 // handles with different layouts share the kernel.
+template <int T, int NG>
+static cudaError_t pipelined_attr(bool hot) {
+  return hot ? cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin())
+             : cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+}
+
 cudaError_t configure_kernels(const View& v) {
   if (!pipelined_matvec_available(v)) return cudaSuccess;
-  if (v.T == 256)
-    return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
-  if (v.T == 192)
-    return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<192, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
-  return cudaFuncSetAttribute(schur_matvec_pipelined_kernel<128, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+  const bool hot = v.num_hot > 0;
+  if (v.T == 256) return pipelined_attr<256, 3>(hot);
+  if (v.T == 192) return pipelined_attr<192, 4>(hot);
+  return pipelined_attr<128, 6>(hot);
+}
+
+template <int T, int NG>
+static void pipelined_launch(const View& v, const PipeLayout& L, int grid, cudaStream_t s) {
+  if (v.num_hot > 0)
+    schur_matvec_pipelined_kernel<T, NG, true><<<grid, NG * T + 32, L.total, s>>>(v, L);
+  else
+    schur_matvec_pipelined_kernel<T, NG, false><<<grid, NG * T + 32, L.total, s>>>(v, L);
 }
 
 cudaError_t launch_schur_matvec(const View& v, cudaStream_t s) {
   if (!pipelined_matvec_available(v)) return launch_pass<MATVEC>(v, s);
-  const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, smem_optin());
+  const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, v.num_hot, smem_optin());
   const int grid = v.num_tiles < v.num_sms ? v.num_tiles : v.num_sms;
-  if (v.T == 256)
-    schur_matvec_pipelined_kernel<256, 3><<<grid, 3 * 256 + 32, L.total, s>>>(v, L);
-  else if (v.T == 192)
-    schur_matvec_pipelined_kernel<192, 4><<<grid, 4 * 192 + 32, L.total, s>>>(v, L);
-  else
-    schur_matvec_pipelined_kernel<128, 6><<<grid, 6 * 128 + 32, L.total, s>>>(v, L);
+  if (v.T == 256) pipelined_launch<256, 3>(v, L, grid, s);
+  else if (v.T == 192) pipelined_launch<192, 4>(v, L, grid, s);
+  else pipelined_launch<128, 6>(v, L, grid, s);
   return CBA_LAUNCHED();
 }
 

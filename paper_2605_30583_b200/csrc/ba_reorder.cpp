@@ -219,6 +219,23 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
       out->chunk_begin.push_back((int)b);
     }
   out->chunk_begin.push_back((int)n);
+
+  // --- 5. hot cameras: far more observations than the average camera (Zipf popularity).  Their rows of q are
+  // accumulated per CTA in shared memory by the pipelined matvec; every other camera goes straight to L2.
+  out->hot_of_cam.assign(nc > 0 ? nc : 1, -1);
+  out->hot_list.clear();
+  if (nc > 0 && n > 0) {
+    const long long limit = std::max<long long>(8192, 4 * (n / nc));
+    std::vector<std::pair<long long, int>> big;
+    for (int c = 0; c < nc; ++c)
+      if (cptr[c + 1] - cptr[c] > limit) big.push_back({cptr[c + 1] - cptr[c], c});
+    std::sort(big.begin(), big.end(), [](const auto& a, const auto& b) { return a.first > b.first || (a.first == b.first && a.second < b.second); });
+    if ((int)big.size() > kMaxHotCameras) big.resize(kMaxHotCameras);
+    for (size_t i = 0; i < big.size(); ++i) {
+      out->hot_of_cam[big[i].second] = (short)i;
+      out->hot_list.push_back(big[i].second);
+    }
+  }
   return 0;
 }
 
