@@ -74,6 +74,10 @@ def test_linearize_parity(pair, key):
         bad = np.abs(j_g - j_o) > 1e-6 + 1e-5 * np.maximum(np.abs(j_o), row_scale)
         assert not bad.any(), (int(bad.sum()), float(np.max(np.abs(j_g - j_o) / row_scale)))
         assert rel_l2(j_g, j_o) <= 1e-5
+        # the literal per-entry reading (no row scale) is reported too: > 99.9 % of the entries meet it; the rest are
+        # entries that cancel to < 1e-2 of their row's scale (C12)
+        strict = np.abs(j_g - j_o) <= 1e-6 + 1e-5 * np.abs(j_o)
+        assert strict.mean() >= 0.999, float(strict.mean())
 
     assert rel_l2(g.export(pkg.U), o.export(ob.U)) <= 1e-5
     assert rel_l2(g.export(pkg.V), o.export(ob.V)) <= 1e-5
