@@ -932,11 +932,19 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     s += NG;
     while (s >= L.stages) { s -= L.stages; ++round; }
   }
-  // p.q: one fp64 atomic per warp
+  // p.q: one fp64 atomic per CTA (same-address atomics serialise in L2: 3,552 per-warp ones would trail the kernel)
   const double tot = warp_sum(dot_part);
-  if (lane == 0) atomicAdd(&v.pcg->pq, tot);
-  if (HOT) {  // all consumer groups are done: one RED per hot camera row and CTA
-    group_bar(15, NG * T);
+  double* warp_tot = reinterpret_cast<double*>(rows);  // this warp's scratch row is free now
+  if (lane == 0) warp_tot[0] = tot;
+  group_bar(15, NG * T);  // all consumer groups are done
+  if (tid < 32) {
+    double a = 0.0;
+    for (int w = lane; w < NG * (T / 32); w += 32)
+      a += *reinterpret_cast<const double*>(smem + L.scratch + (size_t)w * kWarpScratchBytes);
+    a = warp_sum(a);
+    if (lane == 0) atomicAdd(&v.pcg->pq, a);
+  }
+  if (HOT) {  // one RED per hot camera row and CTA
     for (int i = tid; i < 9 * v.num_hot; i += NG * T) {
       const double a = hot_acc[i];
       if (a != 0.0) atomicAdd(v.q + 9ll * __ldg(v.hot_list + i / 9) + i % 9, a);
