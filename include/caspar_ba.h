@@ -77,9 +77,12 @@ typedef struct {
 } caspar_ba_step_info;
 
 /* Environment (read once per caspar_ba_create; tuning / test switches, not needed in normal use):
- *   CASPAR_BA_TILE=256|512|1024  force the tile size T (default: chosen from the longest track and N);
+ *   CASPAR_BA_TILE=128|192|256|512|1024  force the tile size T (default 256, doubled until it holds the
+ *                                longest track);
  *   CASPAR_BA_PIPELINE=0         use the one-block-per-tile Schur pass instead of the persistent
- *                                TMA-pipelined matvec kernel. */
+ *                                TMA-pipelined matvec kernel (which serves tiles of <= 256 slots);
+ *   CASPAR_BA_GRAPH=0            (read at the first solve) launch every PCG kernel on its own instead of
+ *                                replaying chunks of 8 iterations as one CUDA graph. */
 
 /* Build a solver for one problem: validates the indices, reorders the observations (sorted by point
  * into tiles of whole points, camera runs contiguous inside a tile), carves the arena.
