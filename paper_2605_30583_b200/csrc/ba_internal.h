@@ -187,6 +187,5 @@ cudaError_t launch_trial_update(const View& v, cudaStream_t s);
 cudaError_t launch_commit(const View& v, cudaStream_t s);
 cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s);
 cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s);
-int kernels_per(const char* op);  // how many kernels each launcher enqueues (for the launch counter)
 
 }  // namespace cba

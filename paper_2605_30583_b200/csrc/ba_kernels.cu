@@ -671,10 +671,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
       "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
-template <int N>
-__device__ __forceinline__ void consumer_bar() {
-  asm volatile("bar.sync 1, %0;" ::"n"(N) : "memory");
-}
 
 struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
   int j, cam, rank, vinv, meta, stage_bytes;
