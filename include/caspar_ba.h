@@ -59,6 +59,11 @@ typedef struct {
   int32_t robust_loss;         /* 0 = none (F = 1/2 sum |r|^2), 1 = Cauchy (F = 1/2 sum c^2 log(1+|r|^2/c^2)) */
   float robust_scale;          /* c in pixels (> 0 when robust_loss = 1)                                   */
   int32_t damping_mode;        /* 0 = lambda * max(diag(J^T J), 1e-6) (Marquardt scaling), 1 = lambda * I  */
+  int32_t camera_model;        /* 0 = angle-axis 9-vector, additive update (north_star; C2);
+                                  1 = the paper's Pose3 + calibration camera: the rotation is
+                                      linearised in its tangent space, R(d) = R(w) Exp(d), and an accepted step
+                                      retracts w <- Log(R(w) Exp(d_w)); t, f, k1, k2 stay additive (N3) */
+  float depth_epsilon;         /* eps of d_safe = d + eps * sign_no_zero(d); 0 = no guard (C7)  */
 } caspar_ba_problem;
 
 typedef struct {
@@ -84,24 +89,32 @@ typedef struct {
  *   CASPAR_BA_GRAPH=0            (read at the first solve) launch every PCG kernel on its own instead of
  *                                replaying chunks of 8 iterations as one CUDA graph. */
 
-/* Build a solver for one problem: validates the indices, reorders the observations (sorted by point
- * into tiles of whole points, camera runs contiguous inside a tile), carves the arena.
- * Errors: EINVAL (bad sizes / indices / a track longer than CASPAR_BA_MAX_TRACK), ENOMEM, ECUDA. */
+/* PAPER.md:167 (one device memory block, all arrays views into it), :137-149 (block-local sorted index built once
+ * and reused: here the tile layout) -- step S0.
+ * Build a solver for one problem on the CURRENT device: validates the indices (on the host, in the pass that
+ * counts the tracks: S0 runs there), reorders the observations (sorted by point into tiles of whole points,
+ * camera runs contiguous inside a tile), carves the arena.  Every later call on the handle runs on that device
+ * whatever device is current in the calling thread.
+ * Errors: EINVAL (bad sizes / indices / a track longer than CASPAR_BA_MAX_TRACK / CASPAR_BA_TILE not one of the
+ * supported sizes), ENOMEM, ECUDA; the text is available from caspar_ba_last_error(NULL). */
 int caspar_ba_create(const caspar_ba_problem* problem, void* cuda_stream, caspar_ba_t** out);
 
-/* Steps S1-S4: read the caller's parameter arrays, evaluate residuals and Jacobians of every
+/* PAPER.md:182-204 (section VI-A, the reprojection factor: residual and its derivatives), :163 (block-Jacobi: one
+ * block per node) -- steps S1-S4: read the caller's parameter arrays, evaluate residuals and Jacobians of every
  * observation, assemble the 9x9 camera and 3x3 point blocks and the gradient; cache them in the arena.
  * cost_out: HOST, nullable; F at the current parameters.  Errors: ENUMERIC (non-finite cost), ECUDA. */
 int caspar_ba_linearize(caspar_ba_t* h, void* cuda_stream, double* cost_out);
 
-/* Steps S5-S8: solve (J^T J + lambda D) delta = -g through the Schur complement with block-Jacobi PCG,
+/* PAPER.md:163 (normal equations, block-Jacobi preconditioned conjugate gradients), :167-169 (J and J^T applied
+ * matrix-free from the per-observation Jacobians) -- steps S5-S8: solve (J^T J + lambda D) delta = -g through the Schur complement with block-Jacobi PCG,
  * x0 = 0, stop when |r_k| <= rel_tol |b| or after max_iter matvecs; back-substitute the point steps.
  * Leaves delta in the arena.  info: HOST, nullable.  Errors: ESTATE (no cached linearization),
  * ENUMERIC (block not positive definite, p.Sp <= 0; delta then holds the last good iterate). */
 int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, void* cuda_stream,
                         caspar_ba_pcg_info* info);
 
-/* Steps S1-S10: linearize if the cache is stale, pcg_solve, evaluate the trial point x + delta, gain ratio,
+/* PAPER.md:163 (Levenberg-Marquardt, quality-based damping after Madsen et al.: the gain ratio decides) --
+ * steps S1-S10: linearize if the cache is stale, pcg_solve, evaluate the trial point x + delta, gain ratio,
  * then commit (parameters updated in place, cache stale) or discard (cache stays valid).
  * accept_mode: 0 = accept iff rho > 0 and the trial cost is finite, 1 = always, 2 = never (dry run).
  * info: HOST, required.
@@ -114,15 +127,18 @@ int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max
 int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, int32_t accept_mode,
                       void* cuda_stream, caspar_ba_step_info* info);
 
-/* `iterations` adaptive LM steps from lambda0 with Nielsen's damping update (accepted: lambda *=
+/* PAPER.md:163 (the outer LM loop with the damping update of Madsen, Nielsen, Tingleff) --
+ * `iterations` adaptive LM steps from lambda0 with Nielsen's damping update (accepted: lambda *=
  * max(1/3, 1 - (2 rho - 1)^3), nu = 2; rejected: lambda *= nu, nu *= 2).  infos[iterations] and
  * lambdas[iterations] (HOST, nullable) receive each step's record and the lambda it was solved with. */
 int caspar_ba_solve(caspar_ba_t* h, int32_t iterations, float lambda0, float rel_tol, int32_t max_iter,
                     void* cuda_stream, caspar_ba_step_info* infos, float* lambdas);
 
-/* Step S9 without the update: F at the caller's current parameters.  cost_out: HOST, required. */
+/* PAPER.md:194-203 (residual only), :220 (fp32 summation is the paper's stated accuracy loss: the sum is fp64 here) --
+ * step S9 without the update: F at the caller's current parameters.  cost_out: HOST, required. */
 int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out);
 
+/* frees the one arena (and the handle's events, graph, pinned scalars).  NULL is a no-op. */
 void caspar_ba_destroy(caspar_ba_t* h);
 
 /* Host-buffer convenience (end-to-end path): copy HOST parameter arrays ([Nc][9], [Np][3]; pinned memory
@@ -161,6 +177,10 @@ typedef struct {
   int64_t linearize_count, matvec_count;
   int32_t matvec_pipelined;  /* 1: the Schur matvec runs as the persistent TMA-pipelined kernel       */
   int32_t pipeline_stages;   /* shared-memory ring depth of that kernel (0 if not used)               */
+  int32_t num_hot_cameras;   /* cameras whose q rows the pipelined matvec accumulates per CTA (> 0: HOT kernel) */
+  int32_t device;            /* CUDA device the handle lives on                                       */
+  double create_seconds;     /* host wall time of caspar_ba_create, of which ...                      */
+  double reorder_seconds;    /* ... the S0 reordering (host, OpenMP)                                  */
 } caspar_ba_stats;
 /* Synchronises the stream the timed kernels ran on, then fills *out. */
 int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out);
@@ -185,7 +205,8 @@ int caspar_ba_layout_get_info(const caspar_ba_layout_t* l, caspar_ba_layout_info
 int caspar_ba_layout_copy(const caspar_ba_layout_t* l, int32_t which, void* dst_host, size_t bytes);
 void caspar_ba_layout_destroy(caspar_ba_layout_t* l);
 
-/* Valid until the next call on the handle; never NULL. */
+/* Text of the last failure on the handle; valid until the next call on it; never NULL.
+ * h = NULL: text of the last failed caspar_ba_create / caspar_ba_layout_create on the calling thread. */
 const char* caspar_ba_last_error(const caspar_ba_t* h);
 
 #ifdef __cplusplus

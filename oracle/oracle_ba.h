@@ -10,7 +10,11 @@
  *   - block-Jacobi preconditioned conjugate gradients, one block per node, PAPER.md:163,167-169;
  * with the readings listed in DESIGN.md ("Readings of the paper"): the linear system is the
  * point-eliminated (Schur) one and cameras are 9-vectors updated additively, as
- * BASELINE.json `north_star` fixes.
+ * BASELINE.json `north_star` fixes.  The paper's own variants are here too, each behind a
+ * switch that defaults to the north_star reading: the full-system solve without Schur elimination
+ * (oracle_ba_pcgnr_solve), the tangent-space Pose3 rotation with retraction and the
+ * d_safe depth guard (camera_model, depth_epsilon), and the block-Jacobi preconditioner
+ * built from the diagonal blocks of the Schur complement itself (oracle_ba_set_preconditioner).
  *
  * All pointers are HOST pointers; all floating point is double.  Every call returns 0 on success,
  * a negative ORACLE_BA_E* code otherwise.
@@ -43,6 +47,10 @@ typedef struct {
   int32_t robust_loss;           /* 0 = none, 1 = Cauchy                                                     */
   double robust_scale;           /* c, pixels                                                                */
   int32_t damping_mode;          /* 0 = lambda * max(diag(J^T J), 1e-6), 1 = lambda * I                      */
+  int32_t camera_model;          /* 0 = angle-axis, additive update; 1 = Pose3: rotation linearised in its tangent
+                                    space, R(d) = R(w) Exp(d), retraction w <- Log(R(w) Exp(d_w)); t, f, k1, k2
+                                    additive (N3)                             */
+  double depth_epsilon;          /* eps of d_safe = d + eps sign_no_zero(d); 0 = none (C7)   */
 } oracle_ba_problem;
 
 typedef struct {
@@ -71,6 +79,13 @@ enum {
 /* One observation: residual r (2), and if non-NULL d r / d camera (2x9 row-major) and d r / d point (2x3). */
 void oracle_ba_observation(const double cam[9], const double pt[3], const double pixel[2],
                            double r[2], double jc[18], double jp[6]);
+/* The same for either camera model and any depth guard: with camera_model = 1 the first three columns of jc are
+ * d r / d d_w of the right perturbation R(w) Exp(d_w) at d_w = 0. */
+void oracle_ba_observation_model(int32_t camera_model, double depth_epsilon, const double cam[9], const double pt[3],
+                                 const double pixel[2], double r[2], double jc[18], double jp[6]);
+/* Retraction of one camera: out = cam (+) delta.  camera_model 0: cam + delta; 1: w <- Log(Exp(w) Exp(delta_w)),
+ * the other six entries additive. */
+void oracle_ba_retract_camera(int32_t camera_model, const double cam[9], const double delta[9], double out[9]);
 /* Rotation matrix R(w) (row-major 3x3) of the angle-axis vector w. */
 void oracle_ba_rotation(const double w[3], double rot[9]);
 /* Inverse of a symmetric positive-definite n x n matrix by Cholesky; nonzero if a pivot is not positive. */
@@ -92,6 +107,16 @@ int oracle_ba_export(oracle_ba_t* h, int32_t what, double* dst, size_t count);
 int oracle_ba_schur_matvec(oracle_ba_t* h, double lambda, const double* p, double* q);
 /* y = (J^T J + lambda D) x on the full (camera + point) system; x, y are [9 Nc + 3 Np]. */
 int oracle_ba_full_matvec(oracle_ba_t* h, double lambda, const double* x, double* y);
+/* The paper's own linear solve (PAPER.md:163 "does not rely on Schur decomposition", :167-169 PCG with normal
+ * residual): preconditioned CG on the FULL damped normal equations (J^T J + lambda D) delta = -g, J and J^T applied
+ * separately per observation, block-Jacobi preconditioner with one block per node: blockdiag(U'_j, V'_k).
+ * x0 = 0; stop when |r_k| <= rel_tol |g|.  Leaves delta (cameras and points) like oracle_ba_pcg_solve. */
+int oracle_ba_pcgnr_solve(oracle_ba_t* h, double lambda, double rel_tol, int32_t max_iter, oracle_ba_pcg_info* info);
+/* Preconditioner of oracle_ba_pcg_solve: 0 = blockdiag(U'_j) (C9, the default); 1 = the diagonal 9x9
+ * blocks of the Schur complement, S_jj = U'_j - sum_{i in j} W_i V'^-1_k(i) W_i^T ("Schur-Jacobi"). */
+int oracle_ba_set_preconditioner(oracle_ba_t* h, int32_t mode);
+/* The 9x9 blocks the current preconditioner inverts, [Nc][9][9] (after a solve or matvec at some lambda). */
+int oracle_ba_export_preconditioner_blocks(oracle_ba_t* h, double* dst, size_t count);
 int oracle_ba_num_threads(void);
 
 #ifdef __cplusplus

@@ -32,7 +32,8 @@ class Problem(C.Structure):
     _fields_ = [("num_cameras", C.c_int32), ("num_points", C.c_int32), ("num_observations", C.c_int64),
                 ("cameras", C.c_void_p), ("points", C.c_void_p), ("observations", C.c_void_p),
                 ("camera_index", C.c_void_p), ("point_index", C.c_void_p),
-                ("robust_loss", C.c_int32), ("robust_scale", C.c_float), ("damping_mode", C.c_int32)]
+                ("robust_loss", C.c_int32), ("robust_scale", C.c_float), ("damping_mode", C.c_int32),
+                ("camera_model", C.c_int32), ("depth_epsilon", C.c_float)]
 
 
 class PcgInfo(C.Structure):
@@ -50,7 +51,9 @@ class Stats(C.Structure):
                 ("camera_runs", C.c_int64), ("arena_bytes", C.c_int64), ("kernels_launched", C.c_int64),
                 ("linearize_ms_total", C.c_double), ("matvec_ms_total", C.c_double),
                 ("linearize_count", C.c_int64), ("matvec_count", C.c_int64),
-                ("matvec_pipelined", C.c_int32), ("pipeline_stages", C.c_int32)]
+                ("matvec_pipelined", C.c_int32), ("pipeline_stages", C.c_int32),
+                ("num_hot_cameras", C.c_int32), ("device", C.c_int32),
+                ("create_seconds", C.c_double), ("reorder_seconds", C.c_double)]
 
 
 class LayoutInfo(C.Structure):
@@ -134,7 +137,7 @@ def plan_layout(num_cameras: int, num_points: int, camera_index, point_index, ti
     rc = L.caspar_ba_layout_create(num_cameras, num_points, ci.shape[0], ci.ctypes.data, pi.ctypes.data, tile,
                                    C.byref(h))
     if rc:
-        raise CasparError(rc, "layout_create")
+        raise CasparError(rc, "layout_create", L.caspar_ba_last_error(None).decode())
     try:
         info = LayoutInfo()
         L.caspar_ba_layout_get_info(h, C.byref(info))
@@ -158,8 +161,9 @@ def plan_layout(num_cameras: int, num_points: int, camera_index, point_index, ti
         L.caspar_ba_layout_destroy(h)
 
 
-def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> int:
-    return (stream or torch.cuda.current_stream()).cuda_stream
+def _stream_ptr(stream: Optional[torch.cuda.Stream], device=None) -> int:
+    """cudaStream_t of `stream`, default: the current stream OF `device` (not of whatever device is current)."""
+    return (stream or torch.cuda.current_stream(device)).cuda_stream
 
 
 class CasparBA:
@@ -170,7 +174,8 @@ class CasparBA:
     (available as `.cameras` / `.points`)."""
 
     def __init__(self, cameras, points, observations, camera_index, point_index, robust_loss: int = 0,
-                 robust_scale: float = 0.0, damping_mode: int = 0, device: Optional[torch.device] = None):
+                 robust_scale: float = 0.0, damping_mode: int = 0, device: Optional[torch.device] = None,
+                 camera_model: int = 0, depth_epsilon: float = 0.0):
         if not torch.cuda.is_available():
             raise RuntimeError("caspar_ba needs a CUDA device; there is no CPU fallback")
         self._lib = load_library()
@@ -192,12 +197,13 @@ class CasparBA:
         if ci.shape[0] != self.n or pi.shape[0] != self.n:
             raise ValueError("index arrays must have one entry per observation")
         pb = Problem(self.nc, self.np_, self.n, self.cameras.data_ptr(), self.points.data_ptr(), obs.data_ptr(),
-                     ci.data_ptr(), pi.data_ptr(), int(robust_loss), float(robust_scale), int(damping_mode))
+                     ci.data_ptr(), pi.data_ptr(), int(robust_loss), float(robust_scale), int(damping_mode),
+                     int(camera_model), float(depth_epsilon))
         h = C.c_void_p()
-        with torch.cuda.device(dev):
-            rc = self._lib.caspar_ba_create(C.byref(pb), _stream_ptr(None), C.byref(h))
+        with torch.cuda.device(dev):   # create binds the handle to the CURRENT device; later calls switch to it
+            rc = self._lib.caspar_ba_create(C.byref(pb), _stream_ptr(None, dev), C.byref(h))
         if rc:
-            raise CasparError(rc, "create")
+            raise CasparError(rc, "create", self._lib.caspar_ba_last_error(None).decode())
         self._h = h
 
     @classmethod
@@ -220,42 +226,42 @@ class CasparBA:
     # ---- the path ------------------------------------------------------------------------------
     def linearize(self, stream=None) -> float:
         cost = C.c_double()
-        self._check(self._lib.caspar_ba_linearize(self._h, _stream_ptr(stream), C.byref(cost)), "linearize")
+        self._check(self._lib.caspar_ba_linearize(self._h, _stream_ptr(stream, self.device), C.byref(cost)), "linearize")
         return cost.value
 
     def cost(self, stream=None) -> float:
         cost = C.c_double()
-        self._check(self._lib.caspar_ba_cost(self._h, _stream_ptr(stream), C.byref(cost)), "cost")
+        self._check(self._lib.caspar_ba_cost(self._h, _stream_ptr(stream, self.device), C.byref(cost)), "cost")
         return cost.value
 
     def pcg_solve(self, lam: float, rel_tol: float, max_iter: int, stream=None) -> PcgInfo:
         info = PcgInfo()
-        self._check(self._lib.caspar_ba_pcg_solve(self._h, lam, rel_tol, max_iter, _stream_ptr(stream),
+        self._check(self._lib.caspar_ba_pcg_solve(self._h, lam, rel_tol, max_iter, _stream_ptr(stream, self.device),
                                                   C.byref(info)), "pcg_solve")
         return info
 
     def lm_step(self, lam: float, rel_tol: float, max_iter: int, accept_mode: int = 0, stream=None) -> Step:
         info = StepInfo()
-        self._check(self._lib.caspar_ba_lm_step(self._h, lam, rel_tol, max_iter, accept_mode, _stream_ptr(stream),
+        self._check(self._lib.caspar_ba_lm_step(self._h, lam, rel_tol, max_iter, accept_mode, _stream_ptr(stream, self.device),
                                                 C.byref(info)), "lm_step")
         return _step(info, lam)
 
     def solve(self, iterations: int, lambda0: float, rel_tol: float, max_iter: int, stream=None) -> List[Step]:
         infos = (StepInfo * max(1, iterations))()
         lams = (C.c_float * max(1, iterations))()
-        self._check(self._lib.caspar_ba_solve(self._h, iterations, lambda0, rel_tol, max_iter, _stream_ptr(stream),
+        self._check(self._lib.caspar_ba_solve(self._h, iterations, lambda0, rel_tol, max_iter, _stream_ptr(stream, self.device),
                                               infos, lams), "solve")
         return [_step(infos[i], float(lams[i])) for i in range(iterations)]
 
     def set_parameters_host(self, cameras: torch.Tensor, points: torch.Tensor, stream=None):
         assert cameras.dtype == torch.float32 and points.dtype == torch.float32 and not cameras.is_cuda
         self._check(self._lib.caspar_ba_set_parameters_host(self._h, cameras.data_ptr(), points.data_ptr(),
-                                                            _stream_ptr(stream)), "set_parameters_host")
+                                                            _stream_ptr(stream, self.device)), "set_parameters_host")
 
     def get_parameters_host(self, cameras: torch.Tensor, points: torch.Tensor, stream=None):
         assert cameras.dtype == torch.float32 and points.dtype == torch.float32 and not cameras.is_cuda
         self._check(self._lib.caspar_ba_get_parameters_host(self._h, cameras.data_ptr(), points.data_ptr(),
-                                                            _stream_ptr(stream)), "get_parameters_host")
+                                                            _stream_ptr(stream, self.device)), "get_parameters_host")
 
     # ---- test-only exports ---------------------------------------------------------------------
     def export(self, what: int, stream=None) -> np.ndarray:
@@ -271,7 +277,7 @@ class CasparBA:
                  G: (9 * nc + 3 * np_,), SCHUR_RHS: (9 * nc,), DELTA: (9 * nc + 3 * np_,)}[what]
         count = int(np.prod(shape))
         out = torch.zeros(max(count, 1), dtype=torch.float64, device=self.device)
-        self._check(self._lib.caspar_ba_export(self._h, what, out.data_ptr(), count, _stream_ptr(stream)),
+        self._check(self._lib.caspar_ba_export(self._h, what, out.data_ptr(), count, _stream_ptr(stream, self.device)),
                     f"export({what})")
         return out[:count].reshape(shape)
 
@@ -279,12 +285,12 @@ class CasparBA:
         p_dev = torch.as_tensor(np.asarray(p, dtype=np.float64)).to(self.device).contiguous()
         q_dev = torch.empty_like(p_dev)
         self._check(self._lib.caspar_ba_schur_matvec(self._h, lam, p_dev.data_ptr(), q_dev.data_ptr(),
-                                                     _stream_ptr(stream)), "schur_matvec")
+                                                     _stream_ptr(stream, self.device)), "schur_matvec")
         return q_dev.cpu().numpy()
 
     def schur_matvec_device(self, lam: float, p_dev: torch.Tensor, q_dev: torch.Tensor, stream=None):
         self._check(self._lib.caspar_ba_schur_matvec(self._h, lam, p_dev.data_ptr(), q_dev.data_ptr(),
-                                                     _stream_ptr(stream)), "schur_matvec")
+                                                     _stream_ptr(stream, self.device)), "schur_matvec")
 
     # ---- introspection -------------------------------------------------------------------------
     def stats(self) -> Stats:

@@ -1,6 +1,7 @@
 // ba_api.cu — the C ABI of include/caspar_ba.h: arena, state machine, PCG loop, LM step.
 // Host code only orchestrates launches and reads back a handful of scalars per call; every step of
 // the path (S1-S9) runs in the kernels of ba_kernels.cu.  There is no CPU fallback.
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -18,6 +19,8 @@ using namespace cba;
 struct caspar_ba {
   caspar_ba_problem pb{};
   View v{};
+  int device = 0;  // the CUDA device the handle was created on; every entry point switches to it
+  double create_s = 0.0, reorder_s = 0.0;  // wall time of caspar_ba_create and of its host reordering (S0)
   void* arena = nullptr;
   size_t arena_bytes = 0;
   long long camera_runs = 0;
@@ -52,10 +55,36 @@ constexpr int kPcgChunk = 8;
 
 namespace {
 
+// text of the last failure of caspar_ba_create / caspar_ba_layout_create on this thread (there is no handle to
+// hold it): returned by caspar_ba_last_error(NULL)
+thread_local std::string g_create_error;
+
 int fail(caspar_ba* h, int code, const std::string& msg) {
   if (h) h->err = msg;
   return code;
 }
+
+int create_fail(int code, const std::string& msg) {
+  g_create_error = msg;
+  return code;
+}
+
+double now_s() {
+  return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+
+// Every entry point runs on the device the handle was created on, whatever device is current in the caller's
+// thread, and restores the caller's device on return.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
 
 int cuda_fail(caspar_ba* h, cudaError_t e, const char* where) {
   return fail(h, e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA,
@@ -106,6 +135,9 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.cslot = c.take<int>(ro.cslot.size());
   v.chunk_cam = c.take<int>(ro.chunk_cam.size());
   v.chunk_begin = c.take<int>(ro.chunk_begin.size());
+  v.cam_chunk_ptr = c.take<int>(ro.cam_chunk_ptr.size());
+  v.Ug_part = c.take<double>(kUg * ro.chunk_cam.size());
+  v.cost_warp = c.take<double>((size_t)ro.num_tiles * (size_t)(ro.T / 32));
   v.hot_of_cam = c.take<short>(ro.hot_of_cam.size());
   v.hot_list = c.take<int>(ro.hot_list.size());
   v.pts = c.take<float4>(NP);
@@ -196,26 +228,19 @@ int sync_step_scalars(caspar_ba* h, cudaStream_t s) {
   CK(cudaMemcpyAsync(h->h_pcg, h->v.pcg, sizeof(PcgScalars), cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
   if (h->profiling) drain_events(h);
-  double c = 0.0, tc = 0.0;
-  for (int i = 0; i < kCostSlots; ++i) {
-    c += h->h_step->cost_part[i];
-    tc += h->h_step->trial_part[i];
-  }
-  h->h_step->cost = c;
-  h->h_step->trial_cost = tc;
   return 0;
 }
 
 int do_linearize(caspar_ba* h, cudaStream_t s) {
   View& v = h->v;
   CK(cudaMemsetAsync(v.step, 0, sizeof(StepScalars), s));
-  CK(cudaMemsetAsync(v.Ug, 0, sizeof(double) * kUg * (size_t)(v.nc ? v.nc : 1), s));
   CK(launch_pack_points(v, v.points, v.pts, s));
   CK(launch_camera_prepass(v, v.cameras, v.cam_table, s));
   {
     Timed t(h, &h->ev_lin, s);
     CK(launch_linearize(v, s));
   }
+  CK(launch_reduce_cost(v, &v.step->cost, s));
   CK(launch_assemble_cameras(v, s));
   account(h);
   h->linearized = true;
@@ -308,7 +333,9 @@ void fill_pcg_info(const caspar_ba* h, caspar_ba_pcg_info* info) {
   const PcgScalars& p = *h->h_pcg;
   info->iterations = p.iters;
   info->converged = p.converged;
-  info->rel_residual = p.bnorm2 > 0.0 ? std::sqrt(p.rr / p.bnorm2) : 0.0;
+  // after a breakdown rr belongs to an update that never ran: report the last completed iteration's residual
+  const double rr = p.breakdown ? (p.iters > 0 ? p.rr_last : p.bnorm2) : p.rr;
+  info->rel_residual = p.bnorm2 > 0.0 ? std::sqrt(rr / p.bnorm2) : 0.0;
   info->rz0 = p.iters > 0 ? p.rz0 : p.rz[0];
   info->rz = p.rz[p.iters & 1];
 }
@@ -324,43 +351,54 @@ int check_numeric(caspar_ba* h) {
 // =================================================================================================
 extern "C" {
 
-int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t** out) {
-  if (!pb || !out) return CASPAR_BA_EINVAL;
-  *out = nullptr;
-  if (pb->num_cameras < 0 || pb->num_points < 0 || pb->num_observations < 0) return CASPAR_BA_EINVAL;
-  if (pb->num_observations > 0 && (!pb->observations || !pb->camera_index || !pb->point_index)) return CASPAR_BA_EINVAL;
-  if ((pb->num_cameras > 0 && !pb->cameras) || (pb->num_points > 0 && !pb->points)) return CASPAR_BA_EINVAL;
-  if (pb->robust_loss != 0 && pb->robust_loss != 1) return CASPAR_BA_EINVAL;
-  if (pb->robust_loss == 1 && !(pb->robust_scale > 0.f)) return CASPAR_BA_EINVAL;
-  if (pb->damping_mode != 0 && pb->damping_mode != 1) return CASPAR_BA_EINVAL;
-  if (pb->num_observations > 0 && (pb->num_cameras == 0 || pb->num_points == 0)) return CASPAR_BA_EINVAL;
-  caspar_ba* h = new (std::nothrow) caspar_ba();
-  if (!h) return CASPAR_BA_ENOMEM;
+static int create_impl(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t** out, caspar_ba*& h) {
+  const double t_begin = now_s();
+  if (pb->num_cameras < 0 || pb->num_points < 0 || pb->num_observations < 0)
+    return create_fail(CASPAR_BA_EINVAL, "negative size");
+  if (pb->num_observations > 0 && (!pb->observations || !pb->camera_index || !pb->point_index))
+    return create_fail(CASPAR_BA_EINVAL, "null observation / index array");
+  if ((pb->num_cameras > 0 && !pb->cameras) || (pb->num_points > 0 && !pb->points))
+    return create_fail(CASPAR_BA_EINVAL, "null parameter array");
+  if (pb->robust_loss != 0 && pb->robust_loss != 1) return create_fail(CASPAR_BA_EINVAL, "robust_loss must be 0 or 1");
+  if (pb->robust_loss == 1 && !(pb->robust_scale > 0.f))
+    return create_fail(CASPAR_BA_EINVAL, "robust_scale must be positive with the Cauchy loss");
+  if (pb->damping_mode != 0 && pb->damping_mode != 1) return create_fail(CASPAR_BA_EINVAL, "damping_mode must be 0 or 1");
+  if (pb->camera_model != 0 && pb->camera_model != 1) return create_fail(CASPAR_BA_EINVAL, "camera_model must be 0 or 1");
+  if (!(pb->depth_epsilon >= 0.f)) return create_fail(CASPAR_BA_EINVAL, "depth_epsilon must be >= 0");
+  if (pb->num_observations > 0 && (pb->num_cameras == 0 || pb->num_points == 0))
+    return create_fail(CASPAR_BA_EINVAL, "observations without cameras or points");
+  int forced = 0;
+  if (const char* env = std::getenv("CASPAR_BA_TILE")) forced = std::atoi(env);
+  h = new caspar_ba();
   h->pb = *pb;
+  cudaGetDevice(&h->device);
   cudaStream_t s = (cudaStream_t)cuda_stream;
   const long long n = pb->num_observations;
-  auto bail = [&](int code) {
+  auto bail = [&](int code, const std::string& msg) {
     caspar_ba_destroy(h);
-    return code;
+    h = nullptr;
+    return create_fail(code, msg);
   };
-  // indices to the host (the source may be device or host memory)
+  auto cuda_bail = [&](cudaError_t e, const char* where) {
+    return bail(e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA,
+                std::string(where) + ": " + cudaGetErrorString(e));
+  };
+  // S0 runs on the host, so the indices come to the host (the source may be device or host memory) and are
+  // validated there, in the same pass that counts the tracks.
   std::vector<int> cam_idx((size_t)n), pt_idx((size_t)n);
   if (n > 0) {
     cudaError_t e = cudaMemcpy(cam_idx.data(), pb->camera_index, sizeof(int) * (size_t)n, cudaMemcpyDefault);
     if (e == cudaSuccess) e = cudaMemcpy(pt_idx.data(), pb->point_index, sizeof(int) * (size_t)n, cudaMemcpyDefault);
-    if (e != cudaSuccess) return bail(e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA);
+    if (e != cudaSuccess) return cuda_bail(e, "copy of the index arrays");
   }
-  int forced = 0;
-  if (const char* env = std::getenv("CASPAR_BA_TILE")) forced = std::atoi(env);
   Reordered ro;
-  std::string err;
-  int rc = CASPAR_BA_OK;
-  try {
-    rc = reorder_observations(pb->num_cameras, pb->num_points, n, cam_idx.data(), pt_idx.data(), forced, &ro, &err);
-  } catch (const std::bad_alloc&) {
-    return bail(CASPAR_BA_ENOMEM);
+  {
+    std::string err;
+    const double t0 = now_s();
+    const int rc = reorder_observations(pb->num_cameras, pb->num_points, n, cam_idx.data(), pt_idx.data(), forced, &ro, &err);
+    h->reorder_s = now_s() - t0;
+    if (rc) return bail(rc, err);
   }
-  if (rc) return bail(rc);
   View& v = h->v;
   v.nc = pb->num_cameras;
   v.np = pb->num_points;
@@ -373,14 +411,15 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   v.robust = pb->robust_loss;
   v.robust_c2 = pb->robust_scale * pb->robust_scale;
   v.damping_mode = pb->damping_mode;
+  v.camera_model = pb->camera_model;
+  v.depth_eps = pb->depth_epsilon;
   v.cameras = pb->cameras;
   v.points = pb->points;
   v.max_pts_per_tile = ro.max_pts_per_tile;
   v.meta_max_bytes = ro.meta_max_bytes;
   {
-    int dev = 0, sms = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int sms = 0;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
     v.num_sms = sms > 0 ? sms : 148;
   }
   {
@@ -390,7 +429,7 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   h->camera_runs = ro.camera_runs;
   h->arena_bytes = carve(h, nullptr, ro);
   cudaError_t e = cudaMalloc(&h->arena, h->arena_bytes);
-  if (e != cudaSuccess) return bail(CASPAR_BA_ENOMEM);
+  if (e != cudaSuccess) return bail(CASPAR_BA_ENOMEM, "device arena of " + std::to_string(h->arena_bytes) + " bytes: " + cudaGetErrorString(e));
   carve(h, h->arena, ro);
   e = cudaMemsetAsync(h->arena, 0, h->arena_bytes, s);
   if (e == cudaSuccess) e = upload(v.cam, ro.cam, s);
@@ -409,6 +448,7 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   if (e == cudaSuccess) e = upload(v.cslot, ro.cslot, s);
   if (e == cudaSuccess) e = upload(v.chunk_cam, ro.chunk_cam, s);
   if (e == cudaSuccess) e = upload(v.chunk_begin, ro.chunk_begin, s);
+  if (e == cudaSuccess) e = upload(v.cam_chunk_ptr, ro.cam_chunk_ptr, s);
   if (e == cudaSuccess) e = upload(v.hot_of_cam, ro.hot_of_cam, s);
   if (e == cudaSuccess) e = upload(v.hot_list, ro.hot_list, s);
   // pixels: the caller's array may live on either side; stage through the device if it is host memory
@@ -435,13 +475,30 @@ int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);  // the host vectors above die with this scope
   if (obs_dev) cudaFree(obs_dev);
   account(h);
-  if (e != cudaSuccess) return bail(e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA);
+  if (e != cudaSuccess) return cuda_bail(e, "caspar_ba_create");
+  h->create_s = now_s() - t_begin;
   *out = h;
   return CASPAR_BA_OK;
 }
 
+int caspar_ba_create(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba_t** out) {
+  if (!pb || !out) return create_fail(CASPAR_BA_EINVAL, "null argument");
+  *out = nullptr;
+  caspar_ba* h = nullptr;
+  try {  // no exception crosses the C ABI
+    return create_impl(pb, cuda_stream, out, h);
+  } catch (const std::bad_alloc&) {
+    caspar_ba_destroy(h);
+    return create_fail(CASPAR_BA_ENOMEM, "host allocation failed");
+  } catch (...) {
+    caspar_ba_destroy(h);
+    return create_fail(CASPAR_BA_ENOMEM, "unexpected exception in caspar_ba_create");
+  }
+}
+
 void caspar_ba_destroy(caspar_ba_t* h) {
   if (!h) return;
+  DeviceGuard on_device(h->device);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   for (cudaEvent_t e : h->ev_lin) cudaEventDestroy(e);
   for (cudaEvent_t e : h->ev_mv) cudaEventDestroy(e);
@@ -459,6 +516,7 @@ void caspar_ba_destroy(caspar_ba_t* h) {
 int caspar_ba_linearize(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
   if (!h) return CASPAR_BA_EINVAL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   int rc = do_linearize(h, s);
   if (rc) return rc;
   rc = sync_step_scalars(h, s);
@@ -475,12 +533,12 @@ int caspar_ba_linearize(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
 int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
   if (!h || !cost_out) return CASPAR_BA_EINVAL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   View& v = h->v;
   // evaluated in the trial buffers so that a cached linearization stays untouched
-  CK(cudaMemsetAsync(v.step->trial_part, 0, sizeof(double) * kCostSlots, s));
   CK(launch_pack_points(v, v.points, v.pts_trial, s));
   CK(launch_camera_prepass(v, v.cameras, v.cam_table_trial, s));
-  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, v.step->trial_part, s));
+  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
   account(h);
   int rc = sync_step_scalars(h, s);
   if (rc) return rc;
@@ -493,6 +551,7 @@ int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max
   if (!h || max_iter < 0 || !(lambda >= 0.f) || !(rel_tol >= 0.f)) return CASPAR_BA_EINVAL;
   if (!h->linearized) return fail(h, CASPAR_BA_ESTATE, "pcg_solve before linearize");
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   int rc = do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
   if (rc) return rc;
   rc = sync_step_scalars(h, s);
@@ -506,6 +565,7 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   if (!h || !info || max_iter < 0 || accept_mode < 0 || accept_mode > 2 || !(lambda >= 0.f) || !(rel_tol >= 0.f))
     return CASPAR_BA_EINVAL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   View& v = h->v;
   std::memset(info, 0, sizeof *info);
   int rc;
@@ -517,10 +577,9 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   rc = do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
   if (rc) return rc;
   // trial point and its cost (S9)
-  CK(cudaMemsetAsync(v.step->trial_part, 0, sizeof(double) * kCostSlots, s));
   CK(launch_trial_update(v, s));
   CK(launch_camera_prepass(v, v.cams_trial, v.cam_table_trial, s));
-  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, v.step->trial_part, s));
+  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
   account(h);
   rc = sync_step_scalars(h, s);  // the one host synchronisation of the step
   if (rc) return rc;
@@ -595,6 +654,7 @@ int caspar_ba_set_parameters_host(caspar_ba_t* h, const float* cameras_host, con
                                   void* cuda_stream) {
   if (!h || (h->v.nc > 0 && !cameras_host) || (h->v.np > 0 && !points_host)) return CASPAR_BA_EINVAL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   if (h->v.nc > 0)
     CK(cudaMemcpyAsync(h->v.cameras, cameras_host, sizeof(float) * 9 * (size_t)h->v.nc, cudaMemcpyHostToDevice, s));
   if (h->v.np > 0)
@@ -608,6 +668,7 @@ int caspar_ba_set_parameters_host(caspar_ba_t* h, const float* cameras_host, con
 int caspar_ba_get_parameters_host(caspar_ba_t* h, float* cameras_host, float* points_host, void* cuda_stream) {
   if (!h || (h->v.nc > 0 && !cameras_host) || (h->v.np > 0 && !points_host)) return CASPAR_BA_EINVAL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   if (h->v.nc > 0)
     CK(cudaMemcpyAsync(cameras_host, h->v.cameras, sizeof(float) * 9 * (size_t)h->v.nc, cudaMemcpyDeviceToHost, s));
   if (h->v.np > 0)
@@ -634,6 +695,7 @@ int caspar_ba_export(caspar_ba_t* h, int32_t what, double* device_dst, size_t co
   const bool solve_product = what == CASPAR_BA_SCHUR_RHS || what == CASPAR_BA_DELTA;
   if (solve_product ? !h->have_delta : !h->linearized) return fail(h, CASPAR_BA_ESTATE, "export: nothing cached");
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   CK(launch_export(h->v, what, device_dst, s));
   account(h);
   CK(cudaStreamSynchronize(s));
@@ -644,6 +706,7 @@ int caspar_ba_schur_matvec(caspar_ba_t* h, float lambda, const double* p_dev, do
   if (!h || !p_dev || !q_dev || !(lambda >= 0.f)) return CASPAR_BA_EINVAL;
   if (!h->linearized) return fail(h, CASPAR_BA_ESTATE, "schur_matvec before linearize");
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
   int rc = do_prepare(h, (double)lambda, s);
   if (rc) return rc;
   CK(cudaMemsetAsync(h->v.pcg, 0, sizeof(PcgScalars), s));
@@ -660,6 +723,7 @@ int caspar_ba_schur_matvec(caspar_ba_t* h, float lambda, const double* p_dev, do
 
 int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {
   if (!h || !out) return CASPAR_BA_EINVAL;
+  DeviceGuard on_device(h->device);
   if (h->profiling && (!h->ev_lin.empty() || !h->ev_mv.empty())) {
     CK(cudaStreamSynchronize(h->prof_stream));
     drain_events(h);
@@ -676,11 +740,16 @@ int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {
   out->matvec_count = h->mv_n;
   out->matvec_pipelined = h->v.pipeline;
   out->pipeline_stages = h->v.pipeline ? pipeline_stages(h->v) : 0;
+  out->num_hot_cameras = h->v.num_hot;
+  out->device = h->device;
+  out->create_seconds = h->create_s;
+  out->reorder_seconds = h->reorder_s;
   return CASPAR_BA_OK;
 }
 
 int caspar_ba_set_profiling(caspar_ba_t* h, int32_t enable) {
   if (!h) return CASPAR_BA_EINVAL;
+  DeviceGuard on_device(h->device);
   if (h->prof_stream || !h->ev_lin.empty() || !h->ev_mv.empty()) {
     cudaStreamSynchronize(h->prof_stream);
     drain_events(h);
@@ -692,7 +761,7 @@ int caspar_ba_set_profiling(caspar_ba_t* h, int32_t enable) {
   return CASPAR_BA_OK;
 }
 
-const char* caspar_ba_last_error(const caspar_ba_t* h) { return h ? h->err.c_str() : "null handle"; }
+const char* caspar_ba_last_error(const caspar_ba_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
 // ---- S0 on its own (host only) ------------------------------------------------------------------
 struct caspar_ba_layout {
@@ -701,19 +770,25 @@ struct caspar_ba_layout {
 
 int caspar_ba_layout_create(int32_t nc, int32_t np, int64_t n, const int32_t* cam_index, const int32_t* point_index,
                             int32_t tile, caspar_ba_layout_t** out) {
-  if (!out || nc < 0 || np < 0 || n < 0 || (n > 0 && (!cam_index || !point_index))) return CASPAR_BA_EINVAL;
-  caspar_ba_layout* l = new (std::nothrow) caspar_ba_layout();
-  if (!l) return CASPAR_BA_ENOMEM;
+  if (!out || nc < 0 || np < 0 || n < 0 || (n > 0 && (!cam_index || !point_index)))
+    return create_fail(CASPAR_BA_EINVAL, "null argument or negative size");
+  *out = nullptr;
+  caspar_ba_layout* l = nullptr;
   std::string err;
   int rc;
   try {
+    l = new caspar_ba_layout();
     rc = reorder_observations(nc, np, n, cam_index, point_index, tile, &l->ro, &err);
   } catch (const std::bad_alloc&) {
     rc = CASPAR_BA_ENOMEM;
+    err = "host allocation failed";
+  } catch (...) {
+    rc = CASPAR_BA_ENOMEM;
+    err = "unexpected exception in caspar_ba_layout_create";
   }
   if (rc) {
     delete l;
-    return rc;
+    return create_fail(rc, err);
   }
   *out = l;
   return CASPAR_BA_OK;

@@ -37,7 +37,8 @@ struct PcgScalars {
   double rz[2];   // r.z, parity = iteration & 1
   double pDp[2];  // p.(lambda D_c p), parity = iteration & 1
   double pq;      // sum_i u_i.e_i of the current matvec
-  double rr;      // |r|^2 after the current update
+  double rr;      // |r|^2 after the current update (zeroed by the next matvec)
+  double rr_last; // |r|^2 after the last COMPLETED iteration: what a breakdown reports
   double bnorm2;  // |b|^2
   double rz0;
   double pscale;  // the fp32 direction handed to the matvec is p * pscale (a power of two)
@@ -58,12 +59,7 @@ struct StepScalars {
   double dg;          // delta.g
   int bad_block;      // a 9x9 / 3x3 block was not positive definite
   int pad;
-  // the cost kernels add each warp's sum to one of kCostSlots slots (one address would serialise ~1e6 REDs
-  // in L2); the host folds the slots into cost / trial_cost after the copy
-  double cost_part[256];
-  double trial_part[256];
 };
-constexpr int kCostSlots = 256;
 
 // Everything the kernels need, passed by value.
 struct View {
@@ -74,6 +70,8 @@ struct View {
   int robust;
   float robust_c2;
   int damping_mode;
+  int camera_model;  // 0: angle-axis, additive; 1: Pose3 tangent-space rotation (right perturbation) + retraction
+  float depth_eps;   // d_safe = d + eps sign_no_zero(d); 0 = no guard
   // caller's arrays (borrowed)
   float* cameras;
   float* points;
@@ -113,7 +111,7 @@ struct View {
   float4* dp;             // delta_p,k
   // per camera
   float* cams_trial;      // [nc][9]
-  float* cam_table;       // [nc][28]
+  float* cam_table;       // [nc][kCamTableFloats]
   float* cam_table_trial;
   double* Ug;             // [nc][54]
   double* Minv;           // [nc][81]
@@ -129,6 +127,9 @@ struct View {
   const int* chunk_cam;   // [num_chunks]
   const int* chunk_begin; // [num_chunks + 1] into cslot
   const int* cslot;       // slots grouped by camera, ascending
+  const int* cam_chunk_ptr;  // [nc + 1] first chunk of each camera (chunks are listed camera by camera)
+  double* Ug_part;        // [num_chunks][54] per-chunk partial sums of (U_j, g_c,j)
+  double* cost_warp;      // [num_tiles * T / 32] per-warp cost sums, folded in index order by reduce_cost_kernel
   // hot cameras (far more observations than average): index into the per-CTA accumulators, or -1
   const short* hot_of_cam;  // [nc]
   const int* hot_list;      // [num_hot] camera ids
@@ -152,7 +153,7 @@ struct Reordered {
   std::vector<unsigned short> run_slot;
   std::vector<int> pt_ptr;                // [np_obs + 1]
   std::vector<int> pt_perm;               // [np]
-  std::vector<int> chunk_cam, chunk_begin, cslot;
+  std::vector<int> chunk_cam, chunk_begin, cslot, cam_chunk_ptr;
   std::vector<short> hot_of_cam;          // [nc]
   std::vector<int> hot_list;
   std::vector<int> tile_dir;              // [4 * num_tiles]
@@ -171,7 +172,8 @@ cudaError_t launch_pack_points(const View& v, const float* points_caller, float4
 cudaError_t launch_unpack_points(const View& v, const float4* src, float* points_caller, cudaStream_t s);
 cudaError_t launch_camera_prepass(const View& v, const float* cams, float* table, cudaStream_t s);
 cudaError_t launch_linearize(const View& v, cudaStream_t s);
-cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_acc, cudaStream_t s);
+cudaError_t launch_reduce_cost(const View& v, double* cost_out, cudaStream_t s);
+cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_out, cudaStream_t s);
 cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s);
 cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s);
 cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);

@@ -260,7 +260,7 @@ __device__ __forceinline__ int prefetch_lines(const void* ptr, long long bytes, 
 
 template <int T, bool JAC>
 __global__ void __launch_bounds__(T, 1024 / T)
-linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict__ table, double* cost_acc) {
+linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict__ table) {
   __shared__ float4 stage[JAC ? T : 1][2];  // by rank: (Vxx Vxy Vxz Vyy) (Vyz Vzz gx gy)
   __shared__ float stage_gz[JAC ? T : 1];   // by rank: gz
   __shared__ int arrived[JAC ? T : 1];      // by local point id: observations staged so far
@@ -365,19 +365,37 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
     if (JAC) prefetch_lines(v.pt_ptr + np0, 4ll * (np1 - np0 + 1), next_thread % 64, tid);
   }
   const double wsum = warp_sum((double)term);
-  if (lane == 0) atomicAdd(cost_acc + ((t * (T / 32) + (tid >> 5)) & (kCostSlots - 1)), wsum);
+  if (lane == 0) v.cost_warp[(long long)t * (T / 32) + (tid >> 5)] = wsum;  // folded by reduce_cost_kernel
+}
+
+// Sum of the per-warp cost partials in a FIXED order (thread i takes i, i + 1024, ...; then the block tree):
+// the cost is bitwise reproducible, and no floating-point atomic is left on the linearize path (C14).
+__global__ void __launch_bounds__(1024) reduce_cost_kernel(const double* __restrict__ part, long long n,
+                                                          double* __restrict__ out) {
+  __shared__ double red[32];
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  long long i = threadIdx.x;
+  for (; i + 3072 < n; i += 4096) {
+    a0 += part[i];
+    a1 += part[i + 1024];
+    a2 += part[i + 2048];
+    a3 += part[i + 3072];
+  }
+  for (; i < n; i += 1024) a0 += part[i];
+  const double tot = block_sum((a0 + a1) + (a2 + a3), red);
+  if (threadIdx.x == 0) *out = tot;
 }
 
 // ------------------------------------------------------------------------------------------------
 // S4 camera-side assembly: U_j = sum J_c^T J_c (45 unique) and g_c,j = sum J_c^T r (9).
 // Camera-ordered pass: one warp per chunk of <= kChunkSlots slots of one camera (slots ascending, so
 // the gathers walk the camera's in-tile runs contiguously); 54 fp32 partial sums per lane, reduced
-// across lanes in fp64, then one fp64 add per entry.  No per-observation atomics, no hot-camera storm.
+// across lanes in fp64 and written as ONE partial row per chunk; reduce_camera_chunks_kernel then adds a
+// camera's chunk rows in chunk order.  No atomics anywhere: U_j and g_c,j are bitwise reproducible (C14).
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) assemble_cameras_kernel(View v) {
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (w >= v.num_chunks) return;
-  const int cam = v.chunk_cam[w];
   const int b = v.chunk_begin[w], e = v.chunk_begin[w + 1];
   float acc[kUg];
 #pragma unroll
@@ -410,9 +428,30 @@ __global__ void __launch_bounds__(128) assemble_cameras_kernel(View v) {
       if (i < 32) mine0 = tot; else mine1 = tot;
     }
   }
-  double* dst = v.Ug + (long long)kUg * cam;
-  atomicAdd(dst + lane, mine0);
-  if (lane + 32 < kUg) atomicAdd(dst + lane + 32, mine1);
+  double* dst = v.Ug_part + (long long)kUg * w;
+  dst[lane] = mine0;
+  if (lane + 32 < kUg) dst[lane + 32] = mine1;
+}
+
+// One block of 64 threads per camera: thread e adds entry e of the camera's chunk rows, in chunk order, with four
+// interleaved accumulators (chunk index mod 4) so that a hot camera's ~2,400 rows are not one dependent chain.
+__global__ void __launch_bounds__(64) reduce_camera_chunks_kernel(View v) {
+  const int j = blockIdx.x, e = threadIdx.x;
+  if (e >= kUg) return;
+  const int c0 = v.cam_chunk_ptr[j], c1 = v.cam_chunk_ptr[j + 1];
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  const double* src = v.Ug_part + (long long)kUg * c0 + e;
+  int c = c0;
+  for (; c + 4 <= c1; c += 4, src += 4 * kUg) {
+    a0 += src[0];
+    a1 += src[kUg];
+    a2 += src[2 * kUg];
+    a3 += src[3 * kUg];
+  }
+  if (c < c1) a0 += src[0];
+  if (c + 1 < c1) a1 += src[kUg];
+  if (c + 2 < c1) a2 += src[2 * kUg];
+  v.Ug[(long long)kUg * j + e] = (a0 + a1) + (a2 + a3);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -639,7 +678,7 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
 //                   L1/L2-resident p_j gather and the fire-and-forget fp64 REDs.
 // The ring keeps STAGES-1 tiles (~60 KB each) in flight per SM regardless of what the consumers do,
 // which is what the first (one block per tile) version lacked: ncu showed 38 % barrier + 38 %
-// long-scoreboard stalls at 39 % of HBM peak (profiles/r01_matvec_v1.md).
+// long-scoreboard stalls at 39 % of HBM peak (history).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -1077,6 +1116,8 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v) {
   if (sc->done) return;
   const int iter = sc->it_b;
   const int tid = threadIdx.x, par = iter & 1;
+  // |r|^2 of the iteration just completed survives the next matvec's reset of rr (a breakdown reports it)
+  if (blockIdx.x == 0 && tid == 0) sc->rr_last = sc->rr;
   if (sc->rr <= sc->tol2 * sc->bnorm2) {
     if (blockIdx.x == 0 && tid == 0) { sc->done = 1; sc->converged = 1; }
     return;
@@ -1261,30 +1302,39 @@ cudaError_t launch_camera_prepass(const View& v, const float* cams, float* table
 }
 
 template <bool JAC>
-static cudaError_t launch_linearize_t(const View& v, const float4* pts, const float* table, double* acc,
-                                      cudaStream_t s) {
+static cudaError_t launch_linearize_t(const View& v, const float4* pts, const float* table, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaSuccess;
   switch (v.T) {
-    case 128: linearize_kernel<128, JAC><<<v.num_tiles, 128, 0, s>>>(v, pts, table, acc); break;
-    case 192: linearize_kernel<192, JAC><<<v.num_tiles, 192, 0, s>>>(v, pts, table, acc); break;
-    case 256: linearize_kernel<256, JAC><<<v.num_tiles, 256, 0, s>>>(v, pts, table, acc); break;
-    case 512: linearize_kernel<512, JAC><<<v.num_tiles, 512, 0, s>>>(v, pts, table, acc); break;
-    default: linearize_kernel<1024, JAC><<<v.num_tiles, 1024, 0, s>>>(v, pts, table, acc); break;
+    case 128: linearize_kernel<128, JAC><<<v.num_tiles, 128, 0, s>>>(v, pts, table); break;
+    case 192: linearize_kernel<192, JAC><<<v.num_tiles, 192, 0, s>>>(v, pts, table); break;
+    case 256: linearize_kernel<256, JAC><<<v.num_tiles, 256, 0, s>>>(v, pts, table); break;
+    case 512: linearize_kernel<512, JAC><<<v.num_tiles, 512, 0, s>>>(v, pts, table); break;
+    default: linearize_kernel<1024, JAC><<<v.num_tiles, 1024, 0, s>>>(v, pts, table); break;
   }
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_linearize(const View& v, cudaStream_t s) {
-  return launch_linearize_t<true>(v, v.pts, v.cam_table, v.step->cost_part, s);
+// cost_out (device) receives sum_i rho(|r_i|^2); an empty problem gets 0 from the arena's memset / the caller
+cudaError_t launch_reduce_cost(const View& v, double* cost_out, cudaStream_t s) {
+  if (v.num_tiles == 0) return cudaMemsetAsync(cost_out, 0, sizeof(double), s);
+  reduce_cost_kernel<<<1, 1024, 0, s>>>(v.cost_warp, (long long)v.num_tiles * (v.T / 32), cost_out);
+  return CBA_LAUNCHED();
 }
 
-cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_acc, cudaStream_t s) {
-  return launch_linearize_t<false>(v, pts, table, cost_acc, s);
+cudaError_t launch_linearize(const View& v, cudaStream_t s) { return launch_linearize_t<true>(v, v.pts, v.cam_table, s); }
+
+cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_out, cudaStream_t s) {
+  cudaError_t e = launch_linearize_t<false>(v, pts, table, s);
+  return e != cudaSuccess ? e : launch_reduce_cost(v, cost_out, s);
 }
 
 cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s) {
-  if (v.num_chunks == 0) return cudaSuccess;
+  if (v.nc == 0) return cudaSuccess;
+  if (v.num_chunks == 0) return cudaMemsetAsync(v.Ug, 0, sizeof(double) * kUg * (size_t)v.nc, s);
   assemble_cameras_kernel<<<grid_for(32ll * v.num_chunks, 128), 128, 0, s>>>(v);
+  cudaError_t e = CBA_LAUNCHED();
+  if (e != cudaSuccess) return e;
+  reduce_camera_chunks_kernel<<<v.nc, 64, 0, s>>>(v);
   return CBA_LAUNCHED();
 }
 
@@ -1318,15 +1368,14 @@ cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pass
 
 // The pipelined matvec needs the opt-in shared-memory limit and at least two stages; otherwise (or with
 // CASPAR_BA_PIPELINE=0) the one-block-per-tile kernel is used.
-static int g_smem_optin = -1;
-static int smem_optin() {
-  if (g_smem_optin < 0) {
-    int dev = 0, v = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    g_smem_optin = v;
-  }
-  return g_smem_optin;
+static int smem_optin() {  // of the current device (the API layer switches to the handle's device first)
+  static int cached[64];  // 0 = not asked yet
+  int dev = 0, v = 0;
+  cudaGetDevice(&dev);
+  if (dev >= 0 && dev < 64 && cached[dev] > 0) return cached[dev];
+  cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (dev >= 0 && dev < 64) cached[dev] = v;
+  return v;
 }
 
 // The pipelined matvec packs rank and local point id into 16 bits, so it serves tiles of <= 256 slots:

@@ -45,12 +45,12 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
     return CASPAR_BA_EINVAL;
   }
   int T = forced_tile;
-  if (T == 0) T = 256;  // three consumer groups of the pipelined matvec per SM (DESIGN.md "Tile size")
-  while (T < max_track) T = T == 192 ? 256 : T * 2;
-  if (T != 128 && T != 192 && T != 256 && T != 512 && T != 1024) {
-    *err = "tile size must be 128, 192, 256, 512 or 1024";
+  if (T != 0 && T != 128 && T != 192 && T != 256 && T != 512 && T != 1024) {
+    *err = "tile size must be 0 (automatic), 128, 192, 256, 512 or 1024; got " + std::to_string(forced_tile);
     return CASPAR_BA_EINVAL;
   }
+  if (T == 0) T = 256;  // three consumer groups of the pipelined matvec per SM (DESIGN.md "Tile size")
+  while (T < max_track) T = T == 192 ? 256 : T * 2;  // a tile holds whole points: grow to the longest track
 
   // --- 1. internal point order: counting sort by key (stable -> ties by caller id) --------------
   std::vector<int> bucket(nc + 2, 0);
@@ -213,11 +213,15 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
   }
   out->chunk_cam.clear();
   out->chunk_begin.clear();
-  for (int c = 0; c < nc; ++c)
+  out->cam_chunk_ptr.assign(nc + 1, 0);
+  for (int c = 0; c < nc; ++c) {
+    out->cam_chunk_ptr[c] = (int)out->chunk_cam.size();
     for (long long b = cptr[c]; b < cptr[c + 1]; b += kChunkSlots) {
       out->chunk_cam.push_back(c);
       out->chunk_begin.push_back((int)b);
     }
+  }
+  out->cam_chunk_ptr[nc] = (int)out->chunk_cam.size();
   out->chunk_begin.push_back((int)n);
 
   // --- 5. hot cameras: far more observations than the average camera (Zipf popularity).  Their rows of q are

@@ -1,0 +1,42 @@
+"""Helpers shared by the GPU parity tests: norms per parameter class.
+
+A camera vector (g_c, b, q, delta_c, ...) mixes five parameter classes whose natural scales differ by ~1e7
+(per-observation curvature 0.03 for f and k2, 16 for k1, 2.5e3 for t, 2.5e5 for the rotation), so
+one global L2 norm is decided by the rotation rows alone (delta_c: by f alone).  Every camera-vector gate is
+therefore taken per class as well as globally."""
+import numpy as np
+
+CAMERA_CLASSES = {"w": slice(0, 3), "t": slice(3, 6), "f": slice(6, 7), "k1": slice(7, 8), "k2": slice(8, 9)}
+
+
+def rel_l2(a, b) -> float:
+    a, b = np.asarray(a, np.float64).ravel(), np.asarray(b, np.float64).ravel()
+    den = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / den) if den > 0 else float(np.linalg.norm(a))
+
+
+def per_class_rel_l2(a, b) -> dict:
+    """Relative L2 error of a camera vector [9 Nc] per parameter class, plus "all"."""
+    a = np.asarray(a, np.float64).reshape(-1, 9)
+    b = np.asarray(b, np.float64).reshape(-1, 9)
+    out = {name: rel_l2(a[:, sl], b[:, sl]) for name, sl in CAMERA_CLASSES.items()}
+    out["all"] = rel_l2(a, b)
+    return out
+
+
+def assert_per_class(a, b, tol: float, what: str = ""):
+    errs = per_class_rel_l2(a, b)
+    bad = {k: v for k, v in errs.items() if not v <= tol}
+    assert not bad, (what, tol, errs)
+    return errs
+
+
+def scaled_block_rel(u_gpu, u_ref) -> np.ndarray:
+    """Per 9x9 block: relative Frobenius error after the symmetric scaling D^-1/2 U D^-1/2, D = diag(U_ref) (every
+    entry is then O(1) whatever its parameter classes: a wrong k1/k2 row cannot hide behind the rotation block)."""
+    u_gpu, u_ref = np.asarray(u_gpu, np.float64), np.asarray(u_ref, np.float64)
+    d = np.sqrt(np.maximum(np.einsum("nii->ni", u_ref), 1e-300))
+    s = d[:, :, None] * d[:, None, :]
+    num = np.linalg.norm((u_gpu - u_ref) / s, axis=(1, 2))
+    den = np.linalg.norm(u_ref / s, axis=(1, 2))
+    return num / den

@@ -9,6 +9,9 @@ DESIGN.md C12 / C13 say:
   blocks U, V, gradient: <= 1e-5 (U, V) / 1e-4 (g, Schur rhs: signed sums that cancel) relative in L2
   Schur matvec, PCG step: <= 1e-4 relative in L2, both sides at the SAME iteration count (tol = 0)
   cost after the replayed LM schedule (the oracle's own (lambda_t, accepted_t) sequence): <= 1e-4 relative
+Every camera vector (g_c, b, q, delta_c) is gated PER PARAMETER CLASS (rotation, translation, f, k1, k2 columns) as
+well as globally, and every U_j after the symmetric scaling D^-1/2 U D^-1/2: the classes differ by ~1e7 in scale, so a
+global norm alone is decided by the rotation rows (tests/parity_util.py).
 """
 import numpy as np
 import pytest
@@ -16,6 +19,7 @@ import pytest
 import oracle
 import paper_2605_30583_b200 as pkg
 from oracle import binding as ob
+from parity_util import assert_per_class, per_class_rel_l2, rel_l2, scaled_block_rel
 
 pytestmark = pytest.mark.gpu
 
@@ -29,12 +33,6 @@ SCENES = {
     "large": ("large", dict(grid=(12, 16), num_points=30_000)),
     "skewed": ("skewed", dict(num_cameras=300, num_points=30_000)),
 }
-
-
-def rel_l2(a, b):
-    a, b = np.asarray(a, np.float64).ravel(), np.asarray(b, np.float64).ravel()
-    den = np.linalg.norm(b)
-    return float(np.linalg.norm(a - b) / den) if den > 0 else float(np.linalg.norm(a))
 
 
 @pytest.fixture(scope="module")
@@ -79,10 +77,17 @@ def test_linearize_parity(pair, key):
         strict = np.abs(j_g - j_o) <= 1e-6 + 1e-5 * np.abs(j_o)
         assert strict.mean() >= 0.999, float(strict.mean())
 
-    assert rel_l2(g.export(pkg.U), o.export(ob.U)) <= 1e-5
-    assert rel_l2(g.export(pkg.V), o.export(ob.V)) <= 1e-5
+    u_g, u_o = g.export(pkg.U), o.export(ob.U)
+    assert rel_l2(u_g, u_o) <= 1e-5
+    seen = np.einsum("nii->n", u_o) > 0                                # cameras with observations
+    assert scaled_block_rel(u_g[seen], u_o[seen]).max() <= 1e-5        # every block, every parameter class at O(1)
+    assert np.array_equal(u_g[~seen], u_o[~seen])
+    v_g, v_o = g.export(pkg.V), o.export(ob.V)
+    assert rel_l2(v_g, v_o) <= 1e-5
+    norm_v = np.linalg.norm(v_o, axis=(1, 2))
+    assert (np.linalg.norm(v_g - v_o, axis=(1, 2)) <= 1e-4 * norm_v).all()   # per block (fp32 sums of one track)
     grad_g, grad_o = g.export(pkg.G), o.export(ob.G)
-    assert rel_l2(grad_g[:9 * s.num_cameras], grad_o[:9 * s.num_cameras]) <= 1e-4
+    assert_per_class(grad_g[:9 * s.num_cameras], grad_o[:9 * s.num_cameras], 1e-4, "g_c")
     assert rel_l2(grad_g[9 * s.num_cameras:], grad_o[9 * s.num_cameras:]) <= 1e-4
 
 
@@ -103,7 +108,7 @@ def test_schur_matvec_parity(pair, key, lam):
         if trial == 1:  # a preconditioned direction: what PCG actually feeds the operator
             p = p / np.sqrt(np.maximum(o.export(ob.DAMPING)[:9 * s.num_cameras], 1e-12))
         p = p.astype(np.float32).astype(np.float64)  # the kernel reads p in fp32
-        assert rel_l2(g.schur_matvec(lam, p), o.schur_matvec(lam, p)) <= 1e-4
+        assert_per_class(g.schur_matvec(lam, p), o.schur_matvec(lam, p), 1e-4, f"S p, lambda {lam:g}, trial {trial}")
 
 
 def test_schur_operator_is_symmetric_on_the_gpu(pair):
@@ -121,10 +126,10 @@ def test_pcg_step_parity(pair, key):
     iters = 30
     ig, io = g.pcg_solve(LAM, 0.0, iters), o.pcg_solve(LAM, 0.0, iters)
     assert ig.iterations == io.iterations == iters
-    assert rel_l2(g.export(pkg.SCHUR_RHS), o.export(ob.SCHUR_RHS)) <= 1e-4
+    assert_per_class(g.export(pkg.SCHUR_RHS), o.export(ob.SCHUR_RHS), 1e-4, "Schur rhs")
     d_g, d_o = g.export(pkg.DELTA), o.export(ob.DELTA)
     nc9 = 9 * s.num_cameras
-    assert rel_l2(d_g[:nc9], d_o[:nc9]) <= 1e-4
+    assert_per_class(d_g[:nc9], d_o[:nc9], 1e-4, "delta_c")
     assert rel_l2(d_g[nc9:], d_o[nc9:]) <= 1e-4
     assert abs(ig.rel_residual - io.rel_residual) <= 1e-3 * io.rel_residual + 1e-9
 
@@ -140,46 +145,125 @@ def test_pcg_tolerance_stop_matches_oracle(pair):
 
 
 # ------------------------------------------------------------------ S1-S10 replayed LM schedule
+# DESIGN.md C17: a replayed step is gated at north_star's 1e-4 while the ORACLE's own linear solve is resolved
+# (|r|/|b| <= 1e-2 at the config's cap); past that an unconverged CG iterate is a chaotic function of rounding, and
+# the step is gated at the bound the measured table in DESIGN.md C17 supports (skewed only; every other config
+# stays at 1e-4 for all of its steps).
+RESOLVED = 1e-2
+UNRESOLVED_COST_TOL = {"tiny": 1e-4, "small": 1e-4, "mid": 1e-4, "large": 1e-4, "skewed": 2e-2}
+
+
 @pytest.mark.parametrize("key", list(SCENES))
 def test_lm_schedule_parity(scene_cache, key):
     name, kw = SCENES[key]
     s = scene_cache(name, **kw)
     o = oracle.OracleBA.from_scene(s)
-    # the oracle's own adaptive run fixes (lambda_t, accepted_t).  The tolerance 1e-10 is far below what the
-    # fp32 matvec resolves, so both sides do the same work until the recursive residual is negligible; it only
-    # keeps the converged tail of the schedule from iterating on a residual that underflows (at 1e-125 |b| the
-    # oracle's own p.Sp is 0 and C15 reports a breakdown).  C9: stopping an iteration apart is equally correct.
-    cap = min(s.pcg_max_iter, 40)
-    tol = 1e-10
+    # the oracle's own adaptive run fixes (lambda_t, accepted_t), at the CONFIG's PCG cap.  The tolerance 1e-10 is
+    # far below what the fp32 matvec resolves, so both sides do the same work until the recursive residual is
+    # negligible; it only keeps the converged tail of the schedule from iterating on a residual that underflows (at
+    # 1e-125 |b| the oracle's own p.Sp is 0 and C15 reports a breakdown: C16).  C9: stopping an iteration apart is
+    # equally correct.
+    cap, tol = s.pcg_max_iter, 1e-10
     ref = o.solve(s.lm_iterations, 1e-2, tol, cap)
     g = pkg.CasparBA.from_scene(s)
-    gated = 0
+    rows, all_resolved = [], True
     for t, st in enumerate(ref):
-        # Parity of the replay is defined while the linear solves are RESOLVED (oracle PCG residual <= 1e-2 |b|).
-        # Past that (skewed, lambda < 1e-4: the oracle's own PCG stalls at 0.1-1.0 |b|) the iterate is a
-        # chaotic function of rounding, the fp32 and fp64 trajectories fork, and only validity is checked
-        # (test_skewed_adaptive_run_is_valid); DESIGN.md "PCG at tiny lambda".
-        if key == "skewed" and st.pcg_rel_residual > 1e-2:
-            break
         lam = float(np.float32(st.lam))
         got = g.lm_step(lam, tol, cap, accept_mode=1 if st.accepted else 2)
-        if st.pcg_iterations == cap:
-            assert got.pcg_iterations >= cap - 2
-        else:
-            assert abs(got.pcg_iterations - st.pcg_iterations) <= 5, (t, got.pcg_iterations, st.pcg_iterations)
-        assert abs(got.cost_before - st.cost_before) <= 1e-4 * st.cost_before, (t, got.cost_before, st.cost_before)
-        assert abs(got.cost_after - st.cost_after) <= 1e-4 * st.cost_after, (t, got.cost_after, st.cost_after)
-        if st.model_decrease > 1e-6 * st.cost_before:   # below that, fp32 Jacobians do not resolve it
-            # not a north_star gate: with a barely converged PCG the fp32 and fp64 CG paths differ by ~1e-3
-            # in the step while the cost still agrees to 1e-4
-            assert abs(got.model_decrease - st.model_decrease) <= 1e-2 * abs(st.model_decrease), t
-        gated += 1
-    assert gated == len(ref) if key != "skewed" else gated >= 4, gated
-    if gated == len(ref):
+        resolved = st.pcg_rel_residual <= RESOLVED
+        all_resolved &= resolved
+        bound = 1e-4 if resolved else UNRESOLVED_COST_TOL[key]
+        eb = abs(got.cost_before - st.cost_before) / st.cost_before
+        ea = abs(got.cost_after - st.cost_after) / st.cost_after
+        rows.append((t, lam, st.pcg_iterations, got.pcg_iterations, st.pcg_rel_residual, got.pcg_rel_residual, eb, ea))
+        assert eb <= bound and ea <= bound, rows
+        if resolved:
+            if st.pcg_iterations == cap:
+                assert got.pcg_iterations >= cap - 2
+            else:
+                # C16: 1e-10 is below what the fp32 operator resolves; its recursion needs up to ~10 % more iterations
+                assert abs(got.pcg_iterations - st.pcg_iterations) <= max(5, 0.15 * st.pcg_iterations), rows[-1]
+            if st.model_decrease > 1e-6 * st.cost_before:   # below that, fp32 Jacobians do not resolve it
+                # C18 (not a north_star gate): the fp32 and fp64 CG paths differ by ~1e-3 in a barely converged step
+                assert abs(got.model_decrease - st.model_decrease) <= 1e-2 * abs(st.model_decrease), t
+    _dump_table(f"replay_{key}", rows)
+    if all_resolved:
         cams = g.cameras.cpu().numpy().astype(np.float64)
         assert np.abs(cams - o.cameras).max() <= 1e-4 * np.abs(o.cameras).max()
+        errs = per_class_rel_l2(cams, o.cameras)
+        assert max(errs.values()) <= 1e-4, errs
     g.close()
     o.close()
+
+
+def _dump_table(name, rows):
+    """Measured margins go to gpurun_out/ (scratch that comes back from the GPU box); DESIGN.md quotes them."""
+    import json
+    import os
+    try:
+        out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+        os.makedirs(out, exist_ok=True)
+        with open(os.path.join(out, f"{name}.json"), "w") as fh:
+            json.dump(rows, fh)
+    except OSError:
+        pass
+
+
+# ------------------------------------------------------------------ S10 gain ratio and damping
+@pytest.mark.parametrize("key", ["tiny", "small"])
+def test_gain_ratio_and_damping_sequence_parity(scene_cache, key):
+    """S10: the library's OWN adaptive run (caspar_ba_solve: its gain ratio, its accept rule, its Nielsen update)
+    against the oracle's (oracle_ba_solve), step by step until the two may legitimately fork: a step whose model
+    decrease is below 1e-6 F (rho is then a ratio of rounding errors) or whose rho is within 1e-2 of the accept
+    threshold 0.  Up to there: rho to 1e-3, the same accept decision, lambda_t to 1e-2 (Nielsen's factor is
+    1 - (2 rho - 1)^3: d lambda / lambda <= 6 d rho).  The library's rule (rho > 0 AND F+ < F) and the
+    oracle's (rho > 0) must agree on every such step."""
+    name, kw = SCENES[key]
+    s = scene_cache(name, **kw)
+    o = oracle.OracleBA.from_scene(s)
+    ref = o.solve(s.lm_iterations, 1e-2, s.pcg_rel_tol, s.pcg_max_iter)
+    g = pkg.CasparBA.from_scene(s)
+    got = g.solve(s.lm_iterations, 1e-2, s.pcg_rel_tol, s.pcg_max_iter)
+    compared = 0
+    for t, (a, b) in enumerate(zip(got, ref)):
+        if not (b.model_decrease > 1e-6 * b.cost_before) or abs(b.rho) < 1e-2:
+            break
+        assert abs(a.lam - b.lam) <= 1e-2 * b.lam, (t, a.lam, b.lam)
+        assert abs(a.rho - b.rho) <= 1e-3 * max(1.0, abs(b.rho)), (t, a.rho, b.rho)
+        assert a.accepted == b.accepted, t
+        # the two accept rules, both evaluated on the library's own numbers
+        assert (a.rho > 0.0) == (a.rho > 0.0 and a.cost_after < a.cost_before), t
+        assert abs(a.cost_after - b.cost_after) <= 1e-4 * b.cost_after, t
+        compared += 1
+    assert compared >= 3, compared       # the first steps carry all of the cost decrease
+    g.close()
+    o.close()
+
+
+# ------------------------------------------------------------------ determinism (DESIGN.md C14)
+@pytest.mark.parametrize("key", ["tiny", "mid"])
+def test_linearize_is_bitwise_reproducible(scene_cache, key):
+    """Two linearizations of the same point give the same BITS: residuals, Jacobians, V_k, g_p, U_j, g_c and the cost
+    are all summed in a fixed order (no floating-point atomics on this path).  Also the cheapest race detector for
+    the barrier-free point-side assembly (shared-memory counters + fences).  "mid" is the FULL config (5 M
+    observations, several chunks per camera)."""
+    import torch
+    s = scene_cache(key)
+    g = pkg.CasparBA.from_scene(s)
+    runs = []
+    for rep in range(3):
+        cost = g.linearize()
+        runs.append((cost, [g.export_device(w).clone() for w in (pkg.RESIDUALS, pkg.JC, pkg.JP, pkg.U, pkg.V, pkg.G)]))
+    for cost, arrays in runs[1:]:
+        assert cost == runs[0][0]
+        for a, b in zip(arrays, runs[0][1]):
+            assert torch.equal(a, b)
+    # and a fresh handle (another arena) agrees too
+    g2 = pkg.CasparBA.from_scene(s)
+    assert g2.linearize() == runs[0][0]
+    assert torch.equal(g2.export_device(pkg.U), runs[0][1][3]) and torch.equal(g2.export_device(pkg.G), runs[0][1][5])
+    g2.close()
+    g.close()
 
 
 def test_skewed_adaptive_run_is_valid(scene_cache):
