@@ -18,7 +18,8 @@ class _Problem(C.Structure):
     _fields_ = [("num_cameras", C.c_int32), ("num_points", C.c_int32), ("num_observations", C.c_int64),
                 ("cameras", C.c_void_p), ("points", C.c_void_p), ("observations", C.c_void_p),
                 ("camera_index", C.c_void_p), ("point_index", C.c_void_p),
-                ("robust_loss", C.c_int32), ("robust_scale", C.c_double), ("damping_mode", C.c_int32)]
+                ("robust_loss", C.c_int32), ("robust_scale", C.c_double), ("damping_mode", C.c_int32),
+                ("camera_model", C.c_int32), ("depth_epsilon", C.c_double)]
 
 
 class PcgInfo(C.Structure):
@@ -71,6 +72,14 @@ def lib() -> C.CDLL:
         L.oracle_ba_schur_matvec.argtypes = [vp, C.c_double, vp, vp]
         L.oracle_ba_full_matvec.argtypes = [vp, C.c_double, vp, vp]
         L.oracle_ba_num_threads.restype = C.c_int
+        L.oracle_ba_observation_model.argtypes = [C.c_int32, C.c_double] + [vp] * 6
+        L.oracle_ba_observation_model.restype = None
+        L.oracle_ba_retract_camera.argtypes = [C.c_int32, vp, vp, vp]
+        L.oracle_ba_retract_camera.restype = None
+        L.oracle_ba_pcgnr_solve.argtypes = [vp, C.c_double, C.c_double, C.c_int32, C.POINTER(PcgInfo)]
+        L.oracle_ba_set_preconditioner.argtypes = [vp, C.c_int32]
+        L.oracle_ba_set_linear_solver.argtypes = [vp, C.c_int32]
+        L.oracle_ba_export_preconditioner_blocks.argtypes = [vp, vp, C.c_size_t]
         _lib = L
     return _lib
 
@@ -98,6 +107,22 @@ def observation(cam, pt, pixel, jacobians: bool = True):
     return (r, jc.reshape(2, 9), jp.reshape(2, 3)) if jacobians else r
 
 
+def observation_model(camera_model: int, depth_epsilon: float, cam, pt, pixel, jacobians: bool = True):
+    cam, pt, pixel = _f64(cam), _f64(pt), _f64(pixel)
+    r, jc, jp = np.empty(2), np.empty(18), np.empty(6)
+    lib().oracle_ba_observation_model(int(camera_model), float(depth_epsilon), cam.ctypes.data, pt.ctypes.data,
+                                      pixel.ctypes.data, r.ctypes.data, jc.ctypes.data if jacobians else None,
+                                      jp.ctypes.data if jacobians else None)
+    return (r, jc.reshape(2, 9), jp.reshape(2, 3)) if jacobians else r
+
+
+def retract_camera(camera_model: int, cam, delta) -> np.ndarray:
+    cam, delta = _f64(cam), _f64(delta)
+    out = np.empty(9)
+    lib().oracle_ba_retract_camera(int(camera_model), cam.ctypes.data, delta.ctypes.data, out.ctypes.data)
+    return out
+
+
 def spd_inverse(a) -> Tuple[int, np.ndarray]:
     a = _f64(a)
     n = a.shape[0]
@@ -116,7 +141,7 @@ class OracleBA:
     """fp64 oracle handle.  Takes the (float32) scene arrays, up-casts them to float64 copies it owns."""
 
     def __init__(self, cameras, points, observations, camera_index, point_index, robust_loss: int = 0,
-                 robust_scale: float = 0.0, damping_mode: int = 0):
+                 robust_scale: float = 0.0, damping_mode: int = 0, camera_model: int = 0, depth_epsilon: float = 0.0):
         self.cameras = _f64(cameras).copy().reshape(-1, 9)
         self.points = _f64(points).copy().reshape(-1, 3)
         self.observations = _f64(observations).copy().reshape(-1, 2)
@@ -125,7 +150,7 @@ class OracleBA:
         self.nc, self.np_, self.n = self.cameras.shape[0], self.points.shape[0], self.observations.shape[0]
         pb = _Problem(self.nc, self.np_, self.n, self.cameras.ctypes.data, self.points.ctypes.data,
                       self.observations.ctypes.data, self.camera_index.ctypes.data, self.point_index.ctypes.data,
-                      int(robust_loss), float(robust_scale), int(damping_mode))
+                      int(robust_loss), float(robust_scale), int(damping_mode), int(camera_model), float(depth_epsilon))
         self._h = C.c_void_p()
         rc = lib().oracle_ba_create(C.byref(pb), C.byref(self._h))
         if rc:
@@ -134,10 +159,11 @@ class OracleBA:
 
     @classmethod
     def from_scene(cls, scene, damping_mode: int = 0, robust_loss: Optional[int] = None,
-                   robust_scale: Optional[float] = None) -> "OracleBA":
+                   robust_scale: Optional[float] = None, camera_model: int = 0, depth_epsilon: float = 0.0) -> "OracleBA":
         return cls(scene.cameras, scene.points, scene.observations, scene.camera_index, scene.point_index,
                    scene.robust_loss if robust_loss is None else robust_loss,
-                   scene.robust_scale if robust_scale is None else robust_scale, damping_mode)
+                   scene.robust_scale if robust_scale is None else robust_scale, damping_mode, camera_model,
+                   depth_epsilon)
 
     def close(self):
         if getattr(self, "_h", None) and _lib is not None:   # (_lib is gone at interpreter shutdown)
@@ -164,6 +190,23 @@ class OracleBA:
         info = PcgInfo()
         self._check(lib().oracle_ba_pcg_solve(self._h, lam, rel_tol, max_iter, C.byref(info)), "pcg_solve")
         return info
+
+    def pcgnr_solve(self, lam: float, rel_tol: float, max_iter: int) -> PcgInfo:
+        info = PcgInfo()
+        self._check(lib().oracle_ba_pcgnr_solve(self._h, lam, rel_tol, max_iter, C.byref(info)), "pcgnr_solve")
+        return info
+
+    def set_preconditioner(self, mode: int):
+        self._check(lib().oracle_ba_set_preconditioner(self._h, int(mode)), "set_preconditioner")
+
+    def set_linear_solver(self, mode: int):
+        self._check(lib().oracle_ba_set_linear_solver(self._h, int(mode)), "set_linear_solver")
+
+    def preconditioner_blocks(self) -> np.ndarray:
+        out = np.empty((self.nc, 9, 9))
+        self._check(lib().oracle_ba_export_preconditioner_blocks(self._h, out.ctypes.data, out.size),
+                    "export_preconditioner_blocks")
+        return out
 
     def lm_step(self, lam: float, rel_tol: float, max_iter: int, accept_mode: int = 0) -> Step:
         info = StepInfo()

@@ -8,8 +8,9 @@
  * (the single exception, the scalar cost sum, is an fp64 reduction).
  *
  * Parity pins: tests/test_oracle_*.py (finite differences, scipy rotations, explicit sparse J,
- * dense Cholesky of the full damped system, noise-free convergence, limits).  No part of this file
- * is "parity unpinned".
+ * dense Cholesky of the full damped system, noise-free convergence, limits; for the paper's variants:
+ * finite differences through the retraction, scipy's rotation composition, the diagonal blocks of the dense
+ * Schur complement, the dense solution of the full system).  No part of this file is "parity unpinned".
  */
 #include "oracle_ba.h"
 
@@ -35,6 +36,9 @@ struct oracle_ba {
   int linearized;
   /* damped blocks for the lambda in `prepared_lambda` */
   double *Ud, *Minv, *Vinv; /* [Nc][81], [Nc][81], [Np][9] */
+  double* Pblk;             /* [Nc][81] the blocks the preconditioner inverts (U'_j or S_jj) */
+  int preconditioner;       /* 0 = blockdiag(U'), 1 = diagonal blocks of S */
+  int linear_solver;        /* what oracle_ba_lm_step calls: 0 = Schur PCG, 1 = full-system PCGNR */
   double prepared_lambda;
   int prepared;
   double *b, *delta; /* [9Nc], [9Nc+3Np] */
@@ -85,6 +89,14 @@ void oracle_ba_rotation(const double w[3], double rot[9]) {
 
 void oracle_ba_observation(const double cam[9], const double X[3], const double m[2], double r[2], double jc[18],
                            double jp[6]) {
+  oracle_ba_observation_model(0, 0.0, cam, X, m, r, jc, jp);
+}
+
+/* sign_no_zero(d) = +1 for d >= 0, -1 otherwise */
+static double sign_no_zero(double d) { return d >= 0.0 ? 1.0 : -1.0; }
+
+void oracle_ba_observation_model(int32_t camera_model, double depth_epsilon, const double cam[9], const double X[3],
+                                 const double m[2], double r[2], double jc[18], double jp[6]) {
   const double* w = cam;
   const double* t = cam + 3;
   double f = cam[6], k1 = cam[7], k2 = cam[8];
@@ -93,8 +105,10 @@ void oracle_ba_observation(const double cam[9], const double X[3], const double 
   /* P = R X + t */
   double P[3];
   for (int i = 0; i < 3; ++i) P[i] = R[3 * i] * X[0] + R[3 * i + 1] * X[1] + R[3 * i + 2] * X[2] + t[i];
-  /* p = -P_xy / P_z (no epsilon guard: reading C7) */
-  double p[2] = {-P[0] / P[2], -P[1] / P[2]};
+  /* p = -P_xy / d_safe, d_safe = d + eps sign_no_zero(d), d = P_z; eps = 0 is the north_star
+   * reading C7 (no guard).  d d_safe / d d = 1, so the derivatives below only see d_safe in place of P_z. */
+  double d_safe = P[2] + depth_epsilon * sign_no_zero(P[2]);
+  double p[2] = {-P[0] / d_safe, -P[1] / d_safe};
   double n = p[0] * p[0] + p[1] * p[1];
   double rad = 1.0 + k1 * n + k2 * n * n;
   double uv[2] = {f * rad * p[0], f * rad * p[1]};
@@ -105,8 +119,8 @@ void oracle_ba_observation(const double cam[9], const double X[3], const double 
   /* d uv / d p = f (rad I + (2 k1 + 4 k2 n) p p^T) */
   double c = 2.0 * k1 + 4.0 * k2 * n;
   double duv_dp[4] = {f * (rad + c * p[0] * p[0]), f * c * p[0] * p[1], f * c * p[1] * p[0], f * (rad + c * p[1] * p[1])};
-  /* d p / d P = (-1/P_z) [[1, 0, p_x], [0, 1, p_y]] */
-  double iz = -1.0 / P[2];
+  /* d p / d P = (-1/d_safe) [[1, 0, p_x], [0, 1, p_y]] */
+  double iz = -1.0 / d_safe;
   double dp_dP[6] = {iz, 0.0, iz * p[0], 0.0, iz, iz * p[1]};
   /* A = d uv / d P (2x3) */
   double A[6];
@@ -130,6 +144,13 @@ void oracle_ba_observation(const double cam[9], const double X[3], const double 
       for (int j = 0; j < 3; ++j)
         G[3 * i + j] = a1 * q[i] * w[j] - a * Xx[3 * i + j] + b1 * (w[i] * s - th2 * X[i]) * w[j] +
                        b * ((i == j ? s : 0.0) + w[i] * X[j] - 2.0 * X[i] * w[j]);
+    if (camera_model == 1) {
+      /* Pose3 (PAPER.md:163 "linearization ... in the tangent space"; :184 cam_T_world: sf.Pose3): the rotation is
+       * perturbed on the right, R(d) = R Exp(d), so d(R Exp(d) X)/dd at d = 0 is R d(d x X)/dd = -R [X]x. */
+      for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+          G[3 * i + j] = -(R[3 * i] * Xx[j] + R[3 * i + 1] * Xx[3 + j] + R[3 * i + 2] * Xx[6 + j]);
+    }
     for (int i = 0; i < 2; ++i) {
       double* row = jc + 9 * i;
       for (int j = 0; j < 3; ++j) row[j] = A[3 * i] * G[j] + A[3 * i + 1] * G[3 + j] + A[3 * i + 2] * G[6 + j];
@@ -138,6 +159,41 @@ void oracle_ba_observation(const double cam[9], const double X[3], const double 
       row[7] = f * n * p[i];                                 /* d/dk1 */
       row[8] = f * n * n * p[i];                             /* d/dk2 */
     }
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Retraction ("retraction are performed in the tangent space"; N3)      */
+/* ------------------------------------------------------------------------------------------ */
+/* unit quaternion (w, x, y, z) of the rotation vector v: (cos(th/2), sin(th/2) v/th) */
+static void quat_of_rotvec(const double v[3], double q[4]) {
+  double th2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+  double th = sqrt(th2);
+  double k = th2 < 1e-8 ? 0.5 - th2 / 48.0 : sin(0.5 * th) / th; /* sin(th/2)/th */
+  q[0] = cos(0.5 * th);
+  q[1] = k * v[0]; q[2] = k * v[1]; q[3] = k * v[2];
+}
+
+/* rotation vector of a unit quaternion, angle in [0, pi] */
+static void rotvec_of_quat(const double qin[4], double v[3]) {
+  double q[4] = {qin[0], qin[1], qin[2], qin[3]};
+  if (q[0] < 0.0) for (int i = 0; i < 4; ++i) q[i] = -q[i]; /* same rotation, angle <= pi */
+  double s = sqrt(q[1] * q[1] + q[2] * q[2] + q[3] * q[3]); /* sin(th/2) */
+  double k = s < 1e-8 ? 2.0 / q[0] : 2.0 * atan2(s, q[0]) / s;
+  v[0] = k * q[1]; v[1] = k * q[2]; v[2] = k * q[3];
+}
+
+void oracle_ba_retract_camera(int32_t camera_model, const double cam[9], const double delta[9], double out[9]) {
+  for (int a = 0; a < 9; ++a) out[a] = cam[a] + delta[a];
+  if (camera_model == 1) { /* w <- Log(Exp(w) Exp(delta_w)): quaternion product q(w) q(delta_w) */
+    double a[4], b[4], c[4];
+    quat_of_rotvec(cam, a);
+    quat_of_rotvec(delta, b);
+    c[0] = a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3];
+    c[1] = a[0] * b[1] + a[1] * b[0] + a[2] * b[3] - a[3] * b[2];
+    c[2] = a[0] * b[2] - a[1] * b[3] + a[2] * b[0] + a[3] * b[1];
+    c[3] = a[0] * b[3] + a[1] * b[2] - a[2] * b[1] + a[3] * b[0];
+    rotvec_of_quat(c, out);
   }
 }
 
@@ -210,6 +266,8 @@ int oracle_ba_create(const oracle_ba_problem* pb, oracle_ba_t** out) {
   if ((pb->num_cameras > 0 && !pb->cameras) || (pb->num_points > 0 && !pb->points)) return ORACLE_BA_EINVAL;
   if (pb->robust_loss != 0 && pb->robust_loss != 1) return ORACLE_BA_EINVAL;
   if (pb->robust_loss == 1 && !(pb->robust_scale > 0.0)) return ORACLE_BA_EINVAL;
+  if (pb->camera_model != 0 && pb->camera_model != 1) return ORACLE_BA_EINVAL;
+  if (!(pb->depth_epsilon >= 0.0)) return ORACLE_BA_EINVAL;
   for (int64_t i = 0; i < pb->num_observations; ++i)
     if (pb->camera_index[i] < 0 || pb->camera_index[i] >= pb->num_cameras || pb->point_index[i] < 0 ||
         pb->point_index[i] >= pb->num_points)
@@ -230,13 +288,14 @@ int oracle_ba_create(const oracle_ba_problem* pb, oracle_ba_t** out) {
   h->U = (double*)malloc(nc * 81 * sizeof(double));
   h->Ud = (double*)malloc(nc * 81 * sizeof(double));
   h->Minv = (double*)malloc(nc * 81 * sizeof(double));
+  h->Pblk = (double*)malloc(nc * 81 * sizeof(double));
   h->V = (double*)malloc(np * 9 * sizeof(double));
   h->Vinv = (double*)malloc(np * 9 * sizeof(double));
   h->g = (double*)malloc(nv * sizeof(double));
   h->D = (double*)malloc(nv * sizeof(double));
   h->delta = (double*)calloc(nv, sizeof(double));
   h->b = (double*)malloc(9 * nc * sizeof(double));
-  if (rc || !h->r || !h->jc || !h->jp || !h->U || !h->Ud || !h->Minv || !h->V || !h->Vinv || !h->g || !h->D ||
+  if (rc || !h->r || !h->jc || !h->jp || !h->U || !h->Ud || !h->Minv || !h->Pblk || !h->V || !h->Vinv || !h->g || !h->D ||
       !h->delta || !h->b) {
     oracle_ba_destroy(h);
     return ORACLE_BA_ENOMEM;
@@ -248,7 +307,7 @@ int oracle_ba_create(const oracle_ba_problem* pb, oracle_ba_t** out) {
 void oracle_ba_destroy(oracle_ba_t* h) {
   if (!h) return;
   free(h->cam_ptr); free(h->cam_obs); free(h->pt_ptr); free(h->pt_obs);
-  free(h->r); free(h->jc); free(h->jp); free(h->U); free(h->Ud); free(h->Minv); free(h->V); free(h->Vinv);
+  free(h->r); free(h->jc); free(h->jp); free(h->U); free(h->Ud); free(h->Minv); free(h->Pblk); free(h->V); free(h->Vinv);
   free(h->g); free(h->D); free(h->delta); free(h->b);
   free(h);
 }
@@ -263,8 +322,8 @@ static double cost_at(const oracle_ba_t* h, const double* cams, const double* pt
 #pragma omp parallel for schedule(static) reduction(+ : total)
   for (int64_t i = 0; i < h->n_obs; ++i) {
     double r[2];
-    oracle_ba_observation(cams + 9 * (size_t)h->pb.camera_index[i], pts + 3 * (size_t)h->pb.point_index[i],
-                          h->pb.observations + 2 * i, r, NULL, NULL);
+    oracle_ba_observation_model(h->pb.camera_model, h->pb.depth_epsilon, cams + 9 * (size_t)h->pb.camera_index[i],
+                                pts + 3 * (size_t)h->pb.point_index[i], h->pb.observations + 2 * i, r, NULL, NULL);
     double s = r[0] * r[0] + r[1] * r[1];
     total += robust ? c2 * log1p(s / c2) : s;
   }
@@ -291,8 +350,9 @@ int oracle_ba_linearize(oracle_ba_t* h, double* cost_out) {
     double* r = h->r + 2 * i;
     double* jc = h->jc + 18 * i;
     double* jp = h->jp + 6 * i;
-    oracle_ba_observation(h->pb.cameras + 9 * (size_t)h->pb.camera_index[i],
-                          h->pb.points + 3 * (size_t)h->pb.point_index[i], h->pb.observations + 2 * i, r, jc, jp);
+    oracle_ba_observation_model(h->pb.camera_model, h->pb.depth_epsilon,
+                                h->pb.cameras + 9 * (size_t)h->pb.camera_index[i],
+                                h->pb.points + 3 * (size_t)h->pb.point_index[i], h->pb.observations + 2 * i, r, jc, jp);
     double s = r[0] * r[0] + r[1] * r[1];
     if (robust) {
       /* w = rho'(s) = 1 / (1 + s/c^2); r~ = sqrt(w) r, J~ = sqrt(w) J (first-order reweighting) */
@@ -361,18 +421,38 @@ static int prepare_damped(oracle_ba_t* h, double lambda) {
   if (h->prepared && h->prepared_lambda == lambda) return 0;
   int nc = h->nc, np = h->np, bad = 0;
 #pragma omp parallel for schedule(static) reduction(+ : bad)
-  for (int j = 0; j < nc; ++j) {
-    double* Ud = h->Ud + 81 * (size_t)j;
-    memcpy(Ud, h->U + 81 * (size_t)j, 81 * sizeof(double));
-    for (int a = 0; a < 9; ++a) Ud[9 * a + a] += lambda * h->D[9 * (size_t)j + a];
-    if (oracle_ba_spd_inverse(9, Ud, h->Minv + 81 * (size_t)j)) bad++;
-  }
-#pragma omp parallel for schedule(static) reduction(+ : bad)
   for (int k = 0; k < np; ++k) {
     double Vd[9];
     memcpy(Vd, h->V + 9 * (size_t)k, sizeof Vd);
     for (int a = 0; a < 3; ++a) Vd[3 * a + a] += lambda * h->D[9 * (size_t)nc + 3 * (size_t)k + a];
     if (oracle_ba_spd_inverse(3, Vd, h->Vinv + 9 * (size_t)k)) bad++;
+  }
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : bad)
+  for (int j = 0; j < nc; ++j) {
+    double* Ud = h->Ud + 81 * (size_t)j;
+    double* P = h->Pblk + 81 * (size_t)j;
+    memcpy(Ud, h->U + 81 * (size_t)j, 81 * sizeof(double));
+    for (int a = 0; a < 9; ++a) Ud[9 * a + a] += lambda * h->D[9 * (size_t)j + a];
+    memcpy(P, Ud, 81 * sizeof(double));
+    if (h->preconditioner == 1) {
+      /* Schur-Jacobi: S_jj = U'_j - sum_{i in j} W_i V'^-1_k(i) W_i^T, W_i = J_c,i^T J_p,i (9x3) */
+      for (int64_t e = h->cam_ptr[j]; e < h->cam_ptr[j + 1]; ++e) {
+        int64_t i = h->cam_obs[e];
+        const double* Jc = h->jc + 18 * i;
+        const double* Jp = h->jp + 6 * i;
+        const double* Vi = h->Vinv + 9 * (size_t)h->pb.point_index[i];
+        double W[27], WV[27];
+        for (int a = 0; a < 9; ++a)
+          for (int c = 0; c < 3; ++c) W[3 * a + c] = Jc[a] * Jp[c] + Jc[9 + a] * Jp[3 + c];
+        for (int a = 0; a < 9; ++a)
+          for (int c = 0; c < 3; ++c)
+            WV[3 * a + c] = W[3 * a] * Vi[c] + W[3 * a + 1] * Vi[3 + c] + W[3 * a + 2] * Vi[6 + c];
+        for (int a = 0; a < 9; ++a)
+          for (int c = 0; c < 9; ++c)
+            P[9 * a + c] -= WV[3 * a] * W[3 * c] + WV[3 * a + 1] * W[3 * c + 1] + WV[3 * a + 2] * W[3 * c + 2];
+      }
+    }
+    if (oracle_ba_spd_inverse(9, P, h->Minv + 81 * (size_t)j)) bad++;
   }
   if (bad) return ORACLE_BA_ENUMERIC;
   h->prepared = 1;
@@ -549,6 +629,94 @@ int oracle_ba_pcg_solve(oracle_ba_t* h, double lambda, double rel_tol, int32_t m
 }
 
 /* ------------------------------------------------------------------------------------------ */
+/* N1: the paper's own linear solve, PCG with normal residual on the FULL system, no Schur      */
+/* (PAPER.md:163 "solves the linear normal equations directly", :167-169 PCGNR loop)            */
+/* ------------------------------------------------------------------------------------------ */
+int oracle_ba_pcgnr_solve(oracle_ba_t* h, double lambda, double rel_tol, int32_t max_iter, oracle_ba_pcg_info* info) {
+  if (!h || max_iter < 0) return ORACLE_BA_EINVAL;
+  if (!h->linearized) return ORACLE_BA_ESTATE;
+  int save = h->preconditioner;
+  h->preconditioner = 0; /* one block per node: U'_j for a camera, V'_k for a point */
+  if (save != 0) h->prepared = 0;
+  int rc = prepare_damped(h, lambda);
+  h->preconditioner = save;
+  if (save != 0) h->prepared = 0; /* Minv now holds U'^-1: the next Schur solve rebuilds its own */
+  if (rc) return rc;
+  int nc = h->nc, np = h->np;
+  size_t ncv = 9 * (size_t)nc, n = ncv + 3 * (size_t)np;
+  double* x = h->delta;
+  double* work = (double*)malloc(4 * (n ? n : 1) * sizeof(double));
+  if (!work) return ORACLE_BA_ENOMEM;
+  double *res = work, *z = work + n, *p = work + 2 * n, *q = work + 3 * n;
+#define APPLY_MINV(src, dst)                                                                                      \
+  do {                                                                                                            \
+    for (int j = 0; j < nc; ++j) matvec_n(9, h->Minv + 81 * (size_t)j, (src) + 9 * (size_t)j, (dst) + 9 * (size_t)j); \
+    for (int k = 0; k < np; ++k)                                                                                  \
+      matvec_n(3, h->Vinv + 9 * (size_t)k, (src) + ncv + 3 * (size_t)k, (dst) + ncv + 3 * (size_t)k);               \
+  } while (0)
+  /* textbook PCG (Saad, Alg. 9.1) on A = J^T J + lambda D, right-hand side -g, x0 = 0 */
+  memset(x, 0, n * sizeof(double));
+  for (size_t a = 0; a < n; ++a) res[a] = -h->g[a];
+  APPLY_MINV(res, z);
+  memcpy(p, z, n * sizeof(double));
+  double bnorm = sqrt(dot(res, res, n));
+  double rz = dot(res, z, n), rz0 = rz;
+  int iters = 0, converged = 0, status = 0;
+  double rnorm = bnorm;
+  if (bnorm == 0.0) converged = 1;
+  while (!converged && iters < max_iter) {
+    /* normal-residual form: w = J p per observation, then q = J^T w + lambda D p (J and J^T applied separately) */
+    rc = oracle_ba_full_matvec(h, lambda, p, q);
+    if (rc) { status = rc; break; }
+    ++iters;
+    double pq = dot(p, q, n);
+    if (!(pq > 0.0) || !isfinite(pq)) { status = ORACLE_BA_ENUMERIC; break; } /* C15 */
+    double alpha = rz / pq;
+    for (size_t a = 0; a < n; ++a) { x[a] += alpha * p[a]; res[a] -= alpha * q[a]; }
+    rnorm = sqrt(dot(res, res, n));
+    if (rnorm <= rel_tol * bnorm) { converged = 1; break; }
+    APPLY_MINV(res, z);
+    double rz_new = dot(res, z, n);
+    double beta = rz_new / rz;
+    rz = rz_new;
+    for (size_t a = 0; a < n; ++a) p[a] = z[a] + beta * p[a];
+  }
+#undef APPLY_MINV
+  h->have_delta = 1;
+  memset(h->b, 0, ncv * sizeof(double)); /* no Schur right-hand side on this path */
+  if (info) {
+    info->iterations = iters;
+    info->converged = converged;
+    info->rel_residual = bnorm > 0.0 ? rnorm / bnorm : 0.0;
+    info->rz0 = rz0;
+    info->rz = rz;
+  }
+  free(work);
+  return status;
+}
+
+int oracle_ba_set_preconditioner(oracle_ba_t* h, int32_t mode) {
+  if (!h || (mode != 0 && mode != 1)) return ORACLE_BA_EINVAL;
+  if (mode != h->preconditioner) h->prepared = 0;
+  h->preconditioner = mode;
+  return 0;
+}
+
+int oracle_ba_set_linear_solver(oracle_ba_t* h, int32_t mode) {
+  if (!h || (mode != 0 && mode != 1)) return ORACLE_BA_EINVAL;
+  h->linear_solver = mode;
+  return 0;
+}
+
+int oracle_ba_export_preconditioner_blocks(oracle_ba_t* h, double* dst, size_t count) {
+  if (!h || !dst) return ORACLE_BA_EINVAL;
+  if (!h->prepared) return ORACLE_BA_ESTATE;
+  if (count != 81 * (size_t)h->nc) return ORACLE_BA_EINVAL;
+  memcpy(dst, h->Pblk, count * sizeof(double));
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
 /* O7: one LM step and the adaptive schedule (Madsen, Nielsen, Tingleff 2004, Alg. 3.16)       */
 /* ------------------------------------------------------------------------------------------ */
 int oracle_ba_lm_step(oracle_ba_t* h, double lambda, double rel_tol, int32_t max_iter, int32_t accept_mode,
@@ -561,15 +729,19 @@ int oracle_ba_lm_step(oracle_ba_t* h, double lambda, double rel_tol, int32_t max
   }
   memset(info, 0, sizeof *info);
   info->cost_before = h->cost;
-  rc = oracle_ba_pcg_solve(h, lambda, rel_tol, max_iter, &info->pcg);
+  rc = h->linear_solver == 1 ? oracle_ba_pcgnr_solve(h, lambda, rel_tol, max_iter, &info->pcg)
+                             : oracle_ba_pcg_solve(h, lambda, rel_tol, max_iter, &info->pcg);
   if (rc) return rc;
   int nc = h->nc, np = h->np;
   size_t ncv = 9 * (size_t)nc, npv = 3 * (size_t)np;
   double* cams = (double*)malloc((ncv ? ncv : 1) * sizeof(double));
   double* pts = (double*)malloc((npv ? npv : 1) * sizeof(double));
   if (!cams || !pts) { free(cams); free(pts); return ORACLE_BA_ENOMEM; }
-  /* trial point: additive update on all 9 Nc + 3 Np parameters (reading C2) */
-  for (size_t a = 0; a < ncv; ++a) cams[a] = h->pb.cameras[a] + h->delta[a];
+  /* trial point: additive update on all 9 Nc + 3 Np parameters (reading C2); with the Pose3 camera the rotation
+   * is retracted on its manifold (N3) */
+  for (int j = 0; j < nc; ++j)
+    oracle_ba_retract_camera(h->pb.camera_model, h->pb.cameras + 9 * (size_t)j, h->delta + 9 * (size_t)j,
+                             cams + 9 * (size_t)j);
   for (size_t a = 0; a < npv; ++a) pts[a] = h->pb.points[a] + h->delta[ncv + a];
   double f_new = cost_at(h, cams, pts);
   /* model decrease L(0) - L(delta) = -delta^T g - 1/2 |J delta|^2 (valid for an inexact delta; C11) */

@@ -115,6 +115,8 @@ int oracle_ba_pcgnr_solve(oracle_ba_t* h, double lambda, double rel_tol, int32_t
 /* Preconditioner of oracle_ba_pcg_solve: 0 = blockdiag(U'_j) (C9, the default); 1 = the diagonal 9x9
  * blocks of the Schur complement, S_jj = U'_j - sum_{i in j} W_i V'^-1_k(i) W_i^T ("Schur-Jacobi"). */
 int oracle_ba_set_preconditioner(oracle_ba_t* h, int32_t mode);
+/* Linear solver of oracle_ba_lm_step / oracle_ba_solve: 0 = Schur PCG (default), 1 = oracle_ba_pcgnr_solve. */
+int oracle_ba_set_linear_solver(oracle_ba_t* h, int32_t mode);
 /* The 9x9 blocks the current preconditioner inverts, [Nc][9][9] (after a solve or matvec at some lambda). */
 int oracle_ba_export_preconditioner_blocks(oracle_ba_t* h, double* dst, size_t count);
 int oracle_ba_num_threads(void);
