@@ -86,6 +86,8 @@ typedef struct {
  *                                longest track);
  *   CASPAR_BA_PIPELINE=0         use the one-block-per-tile Schur pass instead of the persistent
  *                                TMA-pipelined matvec kernel (which serves tiles of <= 256 slots);
+ *   CASPAR_BA_LIN_PIPELINE=0     use the one-block-per-tile linearize / cost kernels instead of the persistent
+ *                                TMA-pipelined one (which serves tiles of <= 256 slots);
  *   CASPAR_BA_GRAPH=0            (read at the first solve) launch every PCG kernel on its own instead of
  *                                replaying chunks of 8 iterations as one CUDA graph. */
 
@@ -181,6 +183,8 @@ typedef struct {
   int32_t device;            /* CUDA device the handle lives on                                       */
   double create_seconds;     /* host wall time of caspar_ba_create, of which ...                      */
   double reorder_seconds;    /* ... the S0 reordering (host, OpenMP)                                  */
+  int32_t linearize_pipelined; /* 1: linearize and cost run as the persistent TMA-pipelined kernel      */
+  int32_t reserved;
 } caspar_ba_stats;
 /* Synchronises the stream the timed kernels ran on, then fills *out. */
 int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out);

@@ -53,7 +53,8 @@ class Stats(C.Structure):
                 ("linearize_count", C.c_int64), ("matvec_count", C.c_int64),
                 ("matvec_pipelined", C.c_int32), ("pipeline_stages", C.c_int32),
                 ("num_hot_cameras", C.c_int32), ("device", C.c_int32),
-                ("create_seconds", C.c_double), ("reorder_seconds", C.c_double)]
+                ("create_seconds", C.c_double), ("reorder_seconds", C.c_double),
+                ("linearize_pipelined", C.c_int32), ("reserved", C.c_int32)]
 
 
 class LayoutInfo(C.Structure):

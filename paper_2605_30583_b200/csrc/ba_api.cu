@@ -137,7 +137,7 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.chunk_begin = c.take<int>(ro.chunk_begin.size());
   v.cam_chunk_ptr = c.take<int>(ro.cam_chunk_ptr.size());
   v.Ug_part = c.take<double>(kUg * ro.chunk_cam.size());
-  v.cost_warp = c.take<double>((size_t)ro.num_tiles * (size_t)(ro.T / 32));
+  v.cost_warp = c.take<double>((size_t)ro.num_tiles * (size_t)(ro.T / 32) + 32 * (size_t)v.num_sms);
   v.hot_of_cam = c.take<short>(ro.hot_of_cam.size());
   v.hot_list = c.take<int>(ro.hot_list.size());
   v.pts = c.take<float4>(NP);
@@ -425,6 +425,8 @@ static int create_impl(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba
   {
     const char* env = std::getenv("CASPAR_BA_PIPELINE");  // "0" selects the one-block-per-tile Schur pass
     v.pipeline = (!(env && env[0] == '0') && pipelined_matvec_possible(v)) ? 1 : 0;
+    env = std::getenv("CASPAR_BA_LIN_PIPELINE");  // "0" selects the one-block-per-tile linearize / cost kernels
+    v.lin_pipeline = (!(env && env[0] == '0') && pipelined_linearize_possible(v)) ? 1 : 0;
   }
   h->camera_runs = ro.camera_runs;
   h->arena_bytes = carve(h, nullptr, ro);
@@ -741,6 +743,7 @@ int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {
   out->matvec_pipelined = h->v.pipeline;
   out->pipeline_stages = h->v.pipeline ? pipeline_stages(h->v) : 0;
   out->num_hot_cameras = h->v.num_hot;
+  out->linearize_pipelined = h->v.lin_pipeline;
   out->device = h->device;
   out->create_seconds = h->create_s;
   out->reorder_seconds = h->reorder_s;

@@ -99,6 +99,7 @@ struct View {
   int max_pts_per_tile, meta_max_bytes;
   int num_sms;
   int pipeline;                    // 1: Schur matvec runs as the persistent TMA-pipelined kernel
+  int lin_pipeline;                // 1: linearize / cost run as the persistent TMA-pipelined kernel
   // per internal point
   const int* pt_ptr;      // [np_obs + 1] prefix sum of track lengths
   const int* pt_perm;     // [np] internal -> caller point id
@@ -181,6 +182,7 @@ cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s);
 cudaError_t launch_schur_matvec(const View& v, cudaStream_t s);
 cudaError_t configure_kernels(const View& v);  // once per handle: dynamic shared memory opt-in
 bool pipelined_matvec_possible(const View& v);   // shape / shared-memory check, at create
+bool pipelined_linearize_possible(const View& v);
 bool pipelined_matvec_available(const View& v);  // = v.pipeline
 int pipeline_stages(const View& v);
 cudaError_t launch_pcg_update(const View& v, cudaStream_t s);  // two kernels

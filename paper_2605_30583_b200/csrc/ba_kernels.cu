@@ -53,6 +53,46 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// mbarrier / TMA bulk-copy / named-barrier wrappers (inline PTX) shared by the two persistent kernels
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t"
+      "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar,
+                                         unsigned long long policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
+
+__device__ __forceinline__ void group_bar(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+constexpr int kMaxStages = 12;
+
+// ------------------------------------------------------------------------------------------------
 // S0 helpers: gather the caller's observations into slot order; pack / unpack points
 // ------------------------------------------------------------------------------------------------
 __global__ void gather_observations_kernel(View v, const float* __restrict__ observations, float2* __restrict__ px) {
@@ -134,8 +174,9 @@ struct Projection {
   float R[9];                         // rotation rounded to fp32 (J_p = A R)
 };
 
+// depth_eps: d_safe = d + eps sign_no_zero(d); 0 = the unguarded north_star model (C7).
 __device__ __forceinline__ Projection project(const float4* __restrict__ row, float f, float k1, float k2, float X0,
-                                              float X1, float X2, float2 m) {
+                                              float X1, float X2, float2 m, float depth_eps) {
   const double2* rd = reinterpret_cast<const double2*>(row);
   const double2 a0 = __ldg(rd + 0), a1 = __ldg(rd + 1), a2 = __ldg(rd + 2), a3 = __ldg(rd + 3);
   const double2 a4 = __ldg(rd + 4), a5 = __ldg(rd + 5);  // R0 R1 | R2 R3 | R4 R5 | R6 R7 | R8 C0 | C1 C2
@@ -143,7 +184,8 @@ __device__ __forceinline__ Projection project(const float4* __restrict__ row, fl
   const double P0 = fma(a0.x, d0, fma(a0.y, d1, a1.x * d2));
   const double P1 = fma(a1.y, d0, fma(a2.x, d1, a2.y * d2));
   const double P2 = fma(a3.x, d0, fma(a3.y, d1, a4.x * d2));
-  const double inz = -1.0 / P2;  // one shared reciprocal
+  const double d_safe = P2 + (P2 >= 0.0 ? (double)depth_eps : -(double)depth_eps);
+  const double inz = -1.0 / d_safe;  // one shared reciprocal
   const double px = P0 * inz, py = P1 * inz;
   const double n = fma(px, px, py * py);
   const double rad = fma(n, fma((double)k2, n, (double)k1), 1.0);
@@ -159,14 +201,17 @@ __device__ __forceinline__ Projection project(const float4* __restrict__ row, fl
 }
 
 // Full linearization of one observation: J[0..17] = d r / d camera (2x9 row-major), J[18..23] = d r / d point.
+// camera_model 1 (the paper's Pose3 camera): the rotation columns are the derivative with
+// respect to the right perturbation R Exp(d) at d = 0, d(R Exp(d) X)/dd = -R [X]x, so J_w = -J_p [X]x = X x J_p(row).
 __device__ __forceinline__ void linearize_observation(const float* __restrict__ table, int cam, float X0, float X1,
-                                                      float X2, float2 m, float (&J)[24], float& r0, float& r1) {
+                                                      float X2, float2 m, int camera_model, float depth_eps,
+                                                      float (&J)[24], float& r0, float& r1) {
   const float4* row = reinterpret_cast<const float4*>(table) + 9ll * cam;
   const float4 t6 = __ldg(row + 6), t7 = __ldg(row + 7), t8 = __ldg(row + 8);
   const float f = t6.x, k1 = t6.y, k2 = t6.z, th2 = t6.w;
   const float w0 = t7.x, w1 = t7.y, w2 = t7.z, a = t7.w;
   const float b = t8.x, a1 = t8.y, b1 = t8.z;
-  const Projection pr = project(row, f, k1, k2, X0, X1, X2, m);
+  const Projection pr = project(row, f, k1, k2, X0, X1, X2, m, depth_eps);
   r0 = pr.r0;
   r1 = pr.r1;
   const float px = pr.px, py = pr.py, n = pr.n, rad = pr.rad, inz = pr.inz;
@@ -176,6 +221,32 @@ __device__ __forceinline__ void linearize_observation(const float* __restrict__ 
   const float D00 = fmaf(fc * px, px, fr), D01 = fc * px * py, D11 = fmaf(fc * py, py, fr);
   const float A00 = inz * D00, A01 = inz * D01, A02 = inz * fmaf(D00, px, D01 * py);
   const float A10 = A01, A11 = inz * D11, A12 = inz * fmaf(D01, px, D11 * py);
+  // J_p = A R
+  const float* R = pr.R;
+  J[18] = fmaf(A00, R[0], fmaf(A01, R[3], A02 * R[6]));
+  J[19] = fmaf(A00, R[1], fmaf(A01, R[4], A02 * R[7]));
+  J[20] = fmaf(A00, R[2], fmaf(A01, R[5], A02 * R[8]));
+  J[21] = fmaf(A10, R[0], fmaf(A11, R[3], A12 * R[6]));
+  J[22] = fmaf(A10, R[1], fmaf(A11, R[4], A12 * R[7]));
+  J[23] = fmaf(A10, R[2], fmaf(A11, R[5], A12 * R[8]));
+  J[3] = A00; J[4] = A01; J[5] = A02;
+  J[6] = rad * px;
+  const float fn = f * n;
+  J[7] = fn * px;
+  J[8] = fn * n * px;
+  J[12] = A10; J[13] = A11; J[14] = A12;
+  J[15] = rad * py;
+  J[16] = fn * py;
+  J[17] = fn * n * py;
+  if (camera_model == 1) {  // tangent-space rotation block: X x J_p(row)
+    J[0] = X1 * J[20] - X2 * J[19];
+    J[1] = X2 * J[18] - X0 * J[20];
+    J[2] = X0 * J[19] - X1 * J[18];
+    J[9] = X1 * J[23] - X2 * J[22];
+    J[10] = X2 * J[21] - X0 * J[23];
+    J[11] = X0 * J[22] - X1 * J[21];
+    return;
+  }
   // d(R X)/d w = u w^T + b w X^T + b s I - a [X]x,  u = a1 q + b1 (w s - th2 X) - 2 b X,  q = w x X, s = w.X
   const float q0 = w1 * X2 - w2 * X1, q1 = w2 * X0 - w0 * X2, q2 = w0 * X1 - w1 * X0;
   const float s = fmaf(w0, X0, fmaf(w1, X1, w2 * X2));
@@ -192,33 +263,16 @@ __device__ __forceinline__ void linearize_observation(const float* __restrict__ 
   J[0] = fmaf(A00, G00, fmaf(A01, G10, A02 * G20));
   J[1] = fmaf(A00, G01, fmaf(A01, G11, A02 * G21));
   J[2] = fmaf(A00, G02, fmaf(A01, G12, A02 * G22));
-  J[3] = A00; J[4] = A01; J[5] = A02;
-  J[6] = rad * px;
-  const float fn = f * n;
-  J[7] = fn * px;
-  J[8] = fn * n * px;
   J[9] = fmaf(A10, G00, fmaf(A11, G10, A12 * G20));
   J[10] = fmaf(A10, G01, fmaf(A11, G11, A12 * G21));
   J[11] = fmaf(A10, G02, fmaf(A11, G12, A12 * G22));
-  J[12] = A10; J[13] = A11; J[14] = A12;
-  J[15] = rad * py;
-  J[16] = fn * py;
-  J[17] = fn * n * py;
-  // J_p = A R
-  const float* R = pr.R;
-  J[18] = fmaf(A00, R[0], fmaf(A01, R[3], A02 * R[6]));
-  J[19] = fmaf(A00, R[1], fmaf(A01, R[4], A02 * R[7]));
-  J[20] = fmaf(A00, R[2], fmaf(A01, R[5], A02 * R[8]));
-  J[21] = fmaf(A10, R[0], fmaf(A11, R[3], A12 * R[6]));
-  J[22] = fmaf(A10, R[1], fmaf(A11, R[4], A12 * R[7]));
-  J[23] = fmaf(A10, R[2], fmaf(A11, R[5], A12 * R[8]));
 }
 
 __device__ __forceinline__ void residual_observation(const float* __restrict__ table, int cam, float X0, float X1,
-                                                     float X2, float2 m, float& r0, float& r1) {
+                                                     float X2, float2 m, float depth_eps, float& r0, float& r1) {
   const float4* row = reinterpret_cast<const float4*>(table) + 9ll * cam;
   const float4 t6 = __ldg(row + 6);
-  const Projection pr = project(row, t6.x, t6.y, t6.z, X0, X1, X2, m);
+  const Projection pr = project(row, t6.x, t6.y, t6.z, X0, X1, X2, m, depth_eps);
   r0 = pr.r0;
   r1 = pr.r1;
 }
@@ -307,7 +361,7 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
 #pragma unroll
     for (int i = 0; i < 24; ++i) J[i] = 0.f;
     if (cam >= 0) {
-      linearize_observation(table, cam, X.x, X.y, X.z, m, J, r0, r1);
+      linearize_observation(table, cam, X.x, X.y, X.z, m, v.camera_model, v.depth_eps, J, r0, r1);
       const float s2 = fmaf(r0, r0, r1 * r1);
       if (v.robust) {  // Cauchy: w = 1 / (1 + s/c^2), r~ = sqrt(w) r, J~ = sqrt(w) J
         const float q = s2 / v.robust_c2;
@@ -355,7 +409,7 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
   } else {
     if (cam >= 0) {
       float r0, r1;
-      residual_observation(table, cam, X.x, X.y, X.z, m, r0, r1);
+      residual_observation(table, cam, X.x, X.y, X.z, m, v.depth_eps, r0, r1);
       const float s2 = fmaf(r0, r0, r1 * r1);
       term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
     }
@@ -366,6 +420,204 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
   }
   const double wsum = warp_sum((double)term);
   if (lane == 0) v.cost_warp[(long long)t * (T / 32) + (tid >> 5)] = wsum;  // folded by reduce_cost_kernel
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2 + S3 / S9, pipelined: the same per-observation work as linearize_kernel in a PERSISTENT kernel, one CTA per
+// SM, for tiles of <= 256 slots (the default).  linearize_kernel opens every block with two dependent levels of
+// global-memory latency (slot arrays, then the gathers they address) and ends with its stores draining; ncu
+// (profiles/r01_ncu_linearize.md) showed 4.4 long-scoreboard + 1.0 drain stall cycles per issued instruction at
+// 0.55 of the HBM roofline with clean traffic.  Here
+//   producer warp : one lane streams each tile's inputs (camera ids, pixels, rank | point id, the tile's contiguous
+//                   point range, the rank range of each point) into a ring of shared-memory stages with TMA bulk
+//                   copies, several tiles ahead of the consumers;
+//   consumer groups: NG groups of T threads, each on its own tile: inputs come from shared memory, the stage is
+//                   released as soon as they are in registers, the camera row is gathered through L1/L2, the 24
+//                   Jacobian floats leave as streaming 128-bit stores that nothing waits for (no block exit).
+// Point side as in linearize_kernel (rank-ordered sum by the observation that completes its point), with
+// self-resetting counters (atomicInc wraps at the track length) and ONE group barrier per tile, which only
+// orders the reuse of the staging rows and is hidden by the other groups.  Cost: per-thread fp64 accumulation
+// over the thread's tiles (a fixed order), one partial per warp, folded by reduce_cost_kernel.
+// ------------------------------------------------------------------------------------------------
+struct LinLayout {  // byte offsets inside one stage / inside the dynamic shared memory
+  int cam, px, rank, pts, meta, stage_bytes;
+  int stages, sbuf, sbuf_bytes, bars, total;
+};
+
+__host__ __device__ inline LinLayout lin_layout(int T, int NG, int max_pts, int meta_max, bool jac, int smem_limit) {
+  LinLayout L;
+  auto up = [](int x) { return (x + 127) & ~127; };
+  L.cam = 0;
+  L.px = L.cam + T * 4;
+  L.rank = L.px + T * 8;
+  L.pts = up(L.rank + T * 2);
+  L.meta = up(L.pts + max_pts * 16);
+  L.stage_bytes = up(L.meta + (jac ? meta_max : 0));
+  L.sbuf_bytes = jac ? up(T * 40) : 0;  // per group: float4 stage[T][2], float gz[T], unsigned arrived[T]
+  const int fixed = NG * L.sbuf_bytes + 256;
+  int st = (smem_limit - fixed) / L.stage_bytes;
+  if (st > 8) st = 8;  // 8 tiles of inputs (~50 KB) in flight per SM is far more than the consumers can drain
+  L.stages = st;
+  L.sbuf = L.stages * L.stage_bytes;
+  L.bars = L.sbuf + NG * L.sbuf_bytes;
+  L.total = L.bars + 256;
+  return L;
+}
+
+template <int T, int NG, bool JAC>
+__global__ void __launch_bounds__(NG * T + 32, 1)
+linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* __restrict__ table, LinLayout L) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int tid = threadIdx.x;
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L.bars);
+  unsigned long long* empty = full + kMaxStages;
+  volatile int* seen = reinterpret_cast<volatile int*>(empty + kMaxStages);  // see schur_matvec_pipelined_kernel
+  if (tid == 0) {
+    for (int s = 0; s < L.stages; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, T / 32);  // one group consumes a stage
+      seen[s] = 0;
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (JAC)  // per-point arrival counters of every group start at 0 and reset themselves (atomicInc wraps)
+    for (int i = tid; i < NG * T; i += NG * T + 32)
+      reinterpret_cast<unsigned*>(smem + L.sbuf + (size_t)(i / T) * L.sbuf_bytes + T * 36)[i % T] = 0u;
+  __syncthreads();
+  const int G = gridDim.x;
+
+  if (tid >= NG * T) {
+    // ===== producer warp: one lane issues every copy =====
+    if (tid == NG * T) {
+      unsigned long long pol_stream;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+      int s = 0;
+      unsigned ph = 0;
+      int t = blockIdx.x;
+      int4 d = t < v.num_tiles ? __ldg(v.tile_dir + t) : make_int4(0, 0, 0, 0);
+      for (; t < v.num_tiles; t += G) {
+        const int tn = t + G;
+        const int4 dn = tn < v.num_tiles ? __ldg(v.tile_dir + tn) : make_int4(0, 0, 0, 0);  // prefetch next entry
+        mbar_wait(empty + s, ph ^ 1);
+        unsigned char* st = smem + (size_t)s * L.stage_bytes;
+        const unsigned pts_bytes = (unsigned)d.w * 16u;
+        // the blob's first 16 + 2 (npts + 1) bytes, rounded up to 16: header and the rank range of each point
+        const unsigned meta_bytes = JAC ? (16u + ((2u * (unsigned)(d.w + 1) + 15u) & ~15u)) : 0u;
+        mbar_expect_tx(full + s, (unsigned)(T * 4 + T * 8 + T * 2) + pts_bytes + meta_bytes);
+        const long long slot0 = (long long)t * T;
+        bulk_g2s(st + L.cam, v.cam + slot0, T * 4, full + s, pol_stream);
+        bulk_g2s(st + L.px, v.px + slot0, T * 8, full + s, pol_stream);
+        bulk_g2s(st + L.rank, v.rankpid + slot0, T * 2, full + s, pol_stream);
+        bulk_g2s(st + L.pts, pts + d.z, pts_bytes, full + s, pol_stream);
+        if (JAC) bulk_g2s(st + L.meta, v.tile_meta + 16ll * d.x, meta_bytes, full + s, pol_stream);
+        d = dn;
+        if (++s == L.stages) { s = 0; ph ^= 1; }
+      }
+    }
+    return;
+  }
+
+  // ===== consumers: group g takes every NG-th tile of this CTA's sequence =====
+  const int g = tid / T, gt = tid - g * T;
+  const int bar_id = 1 + g;
+  unsigned char* sb = smem + L.sbuf + (size_t)g * L.sbuf_bytes;
+  float4(*stage)[2] = reinterpret_cast<float4(*)[2]>(sb);         // by rank: (Vxx Vxy Vxz Vyy) (Vyz Vzz gx gy)
+  float* stage_gz = reinterpret_cast<float*>(sb + T * 32);        // by rank: gz
+  unsigned* arrived = reinterpret_cast<unsigned*>(sb + T * 36);   // by local point id
+  double cost_acc = 0.0;
+  int s = g % L.stages;
+  int round = g / L.stages;
+  for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G) {
+    while (seen[s] < round) {
+    }
+    mbar_wait(full + s, (unsigned)(round & 1));
+    if (gt == 0) seen[s] = round + 1;
+    const unsigned char* st = smem + (size_t)s * L.stage_bytes;
+    const int cam = reinterpret_cast<const int*>(st + L.cam)[gt];
+    const unsigned rp = reinterpret_cast<const unsigned short*>(st + L.rank)[gt];
+    const unsigned rank = rp & 255u, pid = rp >> 8;
+    const float2 m = reinterpret_cast<const float2*>(st + L.px)[gt];
+    float4 X = make_float4(0.f, 0.f, 0.f, 0.f);
+    int rb = 0, re = 0;  // rank range of this observation's point
+    int p0 = 0;
+    if (cam >= 0) {
+      X = reinterpret_cast<const float4*>(st + L.pts)[pid];
+      if (JAC) {
+        const unsigned short* pt_start = reinterpret_cast<const unsigned short*>(st + L.meta + 16);
+        rb = pt_start[pid];
+        re = pt_start[pid + 1];
+        p0 = reinterpret_cast<const int*>(st + L.meta)[3];
+      }
+    }
+    // everything this thread needs from the stage is in registers: hand it back to the producer
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(empty + s);
+    const long long slot = (long long)t * T + gt;
+    float term = 0.f;
+    if (JAC) {
+      // all warps of the group are done with the previous tile's staging rows and counters
+      group_bar(bar_id, T);
+      float J[24], r0 = 0.f, r1 = 0.f;
+#pragma unroll
+      for (int i = 0; i < 24; ++i) J[i] = 0.f;
+      if (cam >= 0) {
+        linearize_observation(table, cam, X.x, X.y, X.z, m, v.camera_model, v.depth_eps, J, r0, r1);
+        const float s2 = fmaf(r0, r0, r1 * r1);
+        if (v.robust) {  // Cauchy: w = 1 / (1 + s/c^2), r~ = sqrt(w) r, J~ = sqrt(w) J
+          const float q = s2 / v.robust_c2;
+          const float sw = sqrtf(1.0f / (1.0f + q));
+          term = v.robust_c2 * log1pf(q);
+          r0 *= sw; r1 *= sw;
+#pragma unroll
+          for (int i = 0; i < 24; ++i) J[i] *= sw;
+        } else {
+          term = s2;
+        }
+      }
+      // eager stores: six 128-bit chunk arrays + the residual, streamed past L2's keep set
+#pragma unroll
+      for (int c = 0; c < 6; ++c) __stcs(&v.J[c][slot], make_float4(J[4 * c], J[4 * c + 1], J[4 * c + 2], J[4 * c + 3]));
+      __stcs(&v.res[slot], make_float2(r0, r1));
+      if (cam >= 0) {
+        stage[rank][0] = make_float4(fmaf(J[18], J[18], J[21] * J[21]), fmaf(J[18], J[19], J[21] * J[22]),
+                                     fmaf(J[18], J[20], J[21] * J[23]), fmaf(J[19], J[19], J[22] * J[22]));
+        stage[rank][1] = make_float4(fmaf(J[19], J[20], J[22] * J[23]), fmaf(J[20], J[20], J[23] * J[23]),
+                                     fmaf(J[18], r0, J[21] * r1), fmaf(J[19], r0, J[22] * r1));
+        stage_gz[rank] = fmaf(J[20], r0, J[23] * r1);
+        __threadfence_block();
+        const unsigned last = (unsigned)(re - rb - 1);
+        if (atomicInc(&arrived[pid], last) == last) {  // the counter is back at 0 for the group's next tile
+          __threadfence_block();
+          float2 a0 = make_float2(0.f, 0.f), a1 = a0, b0 = a0, b1 = a0;
+          float gz = 0.f;
+          for (int r = rb; r < re; ++r) {  // rank order: V_k, g_p,k do not depend on the arrival order
+            const float4 x = stage[r][0], y = stage[r][1];
+            const float z = stage_gz[r];
+            a0 = __fadd2_rn(a0, make_float2(x.x, x.y));
+            a1 = __fadd2_rn(a1, make_float2(x.z, x.w));
+            b0 = __fadd2_rn(b0, make_float2(y.x, y.y));
+            b1 = __fadd2_rn(b1, make_float2(y.z, y.w));
+            gz += z;
+          }
+          v.V0[p0 + pid] = make_float4(a0.x, a0.y, a1.x, a1.y);
+          v.V1[p0 + pid] = b0;
+          v.gp[p0 + pid] = make_float4(b1.x, b1.y, gz, 0.f);
+        }
+      }
+    } else {
+      if (cam >= 0) {
+        float r0, r1;
+        residual_observation(table, cam, X.x, X.y, X.z, m, v.depth_eps, r0, r1);
+        const float s2 = fmaf(r0, r0, r1 * r1);
+        term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
+      }
+    }
+    cost_acc += (double)term;
+    s += NG;
+    while (s >= L.stages) { s -= L.stages; ++round; }
+  }
+  const double wsum = warp_sum(cost_acc);
+  if ((tid & 31) == 0) v.cost_warp[blockIdx.x * (NG * (T / 32)) + (tid >> 5)] = wsum;
 }
 
 // Sum of the per-warp cost partials in a FIXED order (thread i takes i, i + 1024, ...; then the block tree):
@@ -680,43 +932,11 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
 // which is what the first (one block per tile) version lacked: ncu showed 38 % barrier + 38 %
 // long-scoreboard stalls at 39 % of HBM peak (history).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t"
-      "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar,
-                                         unsigned long long policy) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
-          smem_u32(dst)),
-      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
-      : "memory");
-}
-
 struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
   int j, cam, rank, vinv, meta, stage_bytes;
   int stages, groups, tbuf, tbuf_bytes, sbuf, sbuf_bytes, scratch, hot, bars, total;
 };
 
-constexpr int kMaxStages = 12;
 constexpr int kWarpScratchBytes = 1408;  // per consumer warp: 9 x 33 floats of products + 32 camera ids
 
 // NG consumer groups of T threads share the ring; each group owns a staging area for the point-side sums
@@ -747,9 +967,6 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   return L;
 }
 
-__device__ __forceinline__ void group_bar(int id, int threads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
-}
 
 template <int T, int NG, bool HOT>
 __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(View v, PipeLayout L) {
@@ -1163,9 +1380,34 @@ __global__ void __launch_bounds__(kPcgThreads) delta_c_kernel(View v) {
 // ------------------------------------------------------------------------------------------------
 // S9 trial point and commit
 // ------------------------------------------------------------------------------------------------
+// Pose3 camera (camera_model 1): w <- Log(Exp(w) Exp(d)) through unit quaternions, fp64.
+__device__ __forceinline__ void quat_of_rotvec(double x, double y, double z, double (&q)[4]) {
+  const double th2 = x * x + y * y + z * z, th = sqrt(th2);
+  const double k = th2 < 1e-8 ? 0.5 - th2 / 48.0 : sin(0.5 * th) / th;
+  q[0] = cos(0.5 * th); q[1] = k * x; q[2] = k * y; q[3] = k * z;
+}
+
+__device__ __forceinline__ double retract_rotation(const float* w, const double* d, int a) {
+  double p[4], q[4], c[4];
+  quat_of_rotvec((double)w[0], (double)w[1], (double)w[2], p);
+  quat_of_rotvec(d[0], d[1], d[2], q);
+  c[0] = p[0] * q[0] - p[1] * q[1] - p[2] * q[2] - p[3] * q[3];
+  c[1] = p[0] * q[1] + p[1] * q[0] + p[2] * q[3] - p[3] * q[2];
+  c[2] = p[0] * q[2] - p[1] * q[3] + p[2] * q[0] + p[3] * q[1];
+  c[3] = p[0] * q[3] + p[1] * q[2] - p[2] * q[1] + p[3] * q[0];
+  if (c[0] < 0.0) { c[0] = -c[0]; c[1] = -c[1]; c[2] = -c[2]; c[3] = -c[3]; }  // same rotation, angle <= pi
+  const double s = sqrt(c[1] * c[1] + c[2] * c[2] + c[3] * c[3]);
+  const double k = s < 1e-8 ? 2.0 / c[0] : 2.0 * atan2(s, c[0]) / s;
+  return k * c[1 + a];
+}
+
 __global__ void trial_update_kernel(View v) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < 9ll * v.nc) v.cams_trial[i] = (float)((double)v.cameras[i] + v.x[i]);
+  if (i < 9ll * v.nc) {
+    const int j = (int)(i / 9), a = (int)(i - 9ll * j);
+    if (v.camera_model == 1 && a < 3) v.cams_trial[i] = (float)retract_rotation(v.cameras + 9ll * j, v.x + 9ll * j, a);
+    else v.cams_trial[i] = (float)((double)v.cameras[i] + v.x[i]);
+  }
   if (i < v.np) {
     const float4 p = v.pts[i], d = v.dp[i];
     v.pts_trial[i] = make_float4(p.x + d.x, p.y + d.y, p.z + d.z, 0.f);
@@ -1301,9 +1543,27 @@ cudaError_t launch_camera_prepass(const View& v, const float* cams, float* table
   return CBA_LAUNCHED();
 }
 
+int smem_optin();
+int pipe_groups(int T);
+
+static bool linearize_pipelined(const View& v) { return v.lin_pipeline != 0 && v.T <= 256 && v.num_tiles > 0; }
+static int linearize_grid(const View& v) { return v.num_tiles < v.num_sms ? v.num_tiles : v.num_sms; }
+
+template <int T, int NG, bool JAC>
+static cudaError_t launch_linearize_pipelined(const View& v, const float4* pts, const float* table, cudaStream_t s) {
+  const LinLayout L = lin_layout(T, NG, v.max_pts_per_tile, v.meta_max_bytes, JAC, smem_optin());
+  linearize_pipelined_kernel<T, NG, JAC><<<linearize_grid(v), NG * T + 32, L.total, s>>>(v, pts, table, L);
+  return CBA_LAUNCHED();
+}
+
 template <bool JAC>
 static cudaError_t launch_linearize_t(const View& v, const float4* pts, const float* table, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaSuccess;
+  if (linearize_pipelined(v)) {
+    if (v.T == 256) return launch_linearize_pipelined<256, 3, JAC>(v, pts, table, s);
+    if (v.T == 192) return launch_linearize_pipelined<192, 4, JAC>(v, pts, table, s);
+    return launch_linearize_pipelined<128, 6, JAC>(v, pts, table, s);
+  }
   switch (v.T) {
     case 128: linearize_kernel<128, JAC><<<v.num_tiles, 128, 0, s>>>(v, pts, table); break;
     case 192: linearize_kernel<192, JAC><<<v.num_tiles, 192, 0, s>>>(v, pts, table); break;
@@ -1317,7 +1577,9 @@ static cudaError_t launch_linearize_t(const View& v, const float4* pts, const fl
 // cost_out (device) receives sum_i rho(|r_i|^2); an empty problem gets 0 from the arena's memset / the caller
 cudaError_t launch_reduce_cost(const View& v, double* cost_out, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaMemsetAsync(cost_out, 0, sizeof(double), s);
-  reduce_cost_kernel<<<1, 1024, 0, s>>>(v.cost_warp, (long long)v.num_tiles * (v.T / 32), cost_out);
+  const long long parts = linearize_pipelined(v) ? (long long)linearize_grid(v) * pipe_groups(v.T) * (v.T / 32)
+                                                 : (long long)v.num_tiles * (v.T / 32);
+  reduce_cost_kernel<<<1, 1024, 0, s>>>(v.cost_warp, parts, cost_out);
   return CBA_LAUNCHED();
 }
 
@@ -1368,7 +1630,7 @@ cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pass
 
 // The pipelined matvec needs the opt-in shared-memory limit and at least two stages; otherwise (or with
 // CASPAR_BA_PIPELINE=0) the one-block-per-tile kernel is used.
-static int smem_optin() {  // of the current device (the API layer switches to the handle's device first)
+int smem_optin() {  // of the current device (the API layer switches to the handle's device first)
   static int cached[64];  // 0 = not asked yet
   int dev = 0, v = 0;
   cudaGetDevice(&dev);
@@ -1380,7 +1642,7 @@ static int smem_optin() {  // of the current device (the API layer switches to t
 
 // The pipelined matvec packs rank and local point id into 16 bits, so it serves tiles of <= 256 slots:
 // T = 256 with three consumer groups (800 threads) or T = 128 with six.  Longer tracks use schur_pass_kernel.
-static int pipe_groups(int T) { return T == 256 ? 3 : (T == 192 ? 4 : 6); }
+int pipe_groups(int T) { return T == 256 ? 3 : (T == 192 ? 4 : 6); }
 
 bool pipelined_matvec_possible(const View& v) {
   if (v.num_tiles == 0 || v.T > 256) return false;
@@ -1401,7 +1663,23 @@ static cudaError_t pipelined_attr(bool hot) {
              : cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
 }
 
+template <int T, int NG>
+static cudaError_t linearize_attr() {
+  cudaError_t e = cudaFuncSetAttribute(linearize_pipelined_kernel<T, NG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(linearize_pipelined_kernel<T, NG, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+}
+
+bool pipelined_linearize_possible(const View& v) {
+  if (v.num_tiles == 0 || v.T > 256) return false;
+  return lin_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, true, smem_optin()).stages >= pipe_groups(v.T) + 1;
+}
+
 cudaError_t configure_kernels(const View& v) {
+  if (linearize_pipelined(v)) {
+    const cudaError_t e = v.T == 256 ? linearize_attr<256, 3>() : (v.T == 192 ? linearize_attr<192, 4>() : linearize_attr<128, 6>());
+    if (e != cudaSuccess) return e;
+  }
   if (!pipelined_matvec_available(v)) return cudaSuccess;
   const bool hot = v.num_hot > 0;
   if (v.T == 256) return pipelined_attr<256, 3>(hot);

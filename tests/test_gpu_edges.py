@@ -145,11 +145,14 @@ def test_every_tile_size_and_both_matvec_kernels(scene_cache, monkeypatch, tile,
     Schur pass and the persistent TMA-pipelined one (tiles of <= 256 slots) must both match the oracle."""
     monkeypatch.setenv("CASPAR_BA_TILE", str(tile))
     monkeypatch.setenv("CASPAR_BA_PIPELINE", pipeline)
+    monkeypatch.setenv("CASPAR_BA_LIN_PIPELINE", pipeline)     # the same choice for linearize / cost
     s = scene_cache("mid", grid=(10, 12), num_points=40_000)
     g = pkg.CasparBA.from_scene(s)
     o = oracle.OracleBA.from_scene(s)
     assert g.stats().tile_slots == tile
     assert g.stats().matvec_pipelined == (1 if pipeline == "1" and tile <= 256 else 0)
+    assert g.stats().linearize_pipelined == (1 if pipeline == "1" and tile <= 256 else 0)
+    assert abs(g.cost() - o.cost()) <= 1e-9 * o.cost()         # the residual-only instantiation
     _step_matches(g, o)
     p = np.random.default_rng(3).normal(size=9 * g.nc).astype(np.float32).astype(np.float64)
     assert rel_l2(g.schur_matvec(LAM, p), o.schur_matvec(LAM, p)) <= 1e-4

@@ -55,7 +55,7 @@ def large(scene_cache):
 
 def test_bench_configuration(large):
     st = large["gpu"].stats()
-    assert st.tile_slots == 256 and st.matvec_pipelined == 1
+    assert st.tile_slots == 256 and st.matvec_pipelined == 1 and st.linearize_pipelined == 1
     assert st.padded_slots >= large["scene"].num_observations
     assert st.padded_slots <= 1.03 * large["scene"].num_observations      # padding of whole-point tiles
 

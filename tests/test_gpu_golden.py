@@ -63,7 +63,7 @@ def full(request, scene_cache):
 
 def test_launch_configuration(full):
     st = full["gpu"].stats()
-    assert st.tile_slots == 256 and st.matvec_pipelined == 1
+    assert st.tile_slots == 256 and st.matvec_pipelined == 1 and st.linearize_pipelined == 1
     if full["name"] == "skewed":
         assert st.num_hot_cameras > 0          # the HOT instantiation of the pipelined matvec
     else:

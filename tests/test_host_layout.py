@@ -145,3 +145,22 @@ def test_binding_refuses_to_run_without_a_gpu():
     s = make_scene("tiny")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         pkg.CasparBA.from_scene(s)
+
+
+@pytest.mark.parametrize("tile", [-1, 1, 3, 6, 100, 2048])
+def test_unsupported_tile_sizes_are_rejected_with_a_message(tile):
+    """A tile request outside {0, 128, 192, 256, 512, 1024} is EINVAL (a negative one used to loop forever), and the
+    text of the failure is available without a handle (caspar_ba_last_error(NULL))."""
+    s = make_scene("tiny")
+    with pytest.raises(pkg.CasparError) as e:
+        pkg.plan_layout(s.num_cameras, s.num_points, s.camera_index, s.point_index, tile=tile)
+    assert e.value.code == -1 and "tile size" in str(e.value) and str(tile) in str(e.value)
+
+
+def test_layout_errors_carry_their_text():
+    s = make_scene("tiny")
+    bad = s.camera_index.copy()
+    bad[17] = s.num_cameras
+    with pytest.raises(pkg.CasparError) as e:
+        pkg.plan_layout(s.num_cameras, s.num_points, bad, s.point_index)
+    assert e.value.code == -1 and "out of range at observation 17" in str(e.value)
