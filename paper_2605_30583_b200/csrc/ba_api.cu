@@ -240,7 +240,7 @@ int do_linearize(caspar_ba* h, cudaStream_t s) {
     Timed t(h, &h->ev_lin, s);
     CK(launch_linearize(v, s));
   }
-  CK(launch_reduce_cost(v, &v.step->cost, s));
+  CK(launch_linearize_cost(v, &v.step->cost, s));
   CK(launch_assemble_cameras(v, s));
   account(h);
   h->linearized = true;

@@ -423,8 +423,10 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
 }
 
 // ------------------------------------------------------------------------------------------------
-// S2 + S3 / S9, pipelined: the same per-observation work as linearize_kernel in a PERSISTENT kernel, one CTA per
-// SM, for tiles of <= 256 slots (the default).  linearize_kernel opens every block with two dependent levels of
+// S2 + S3, pipelined: the same per-observation work as linearize_kernel in a PERSISTENT kernel, one CTA per
+// SM, for tiles of <= 256 slots (the default).  (Only JAC = true is launched.  The residual-only cost pass S9 stays
+// on linearize_kernel<T, false>: it has a quarter of the instructions and nothing to overlap them with, so it wants
+// the 40 resident warps of five small blocks, not the 24 of one 800-thread CTA: 0.32 ms against 0.42 ms measured.)  linearize_kernel opens every block with two dependent levels of
 // global-memory latency (slot arrays, then the gathers they address) and ends with its stores draining; ncu
 // (profiles/r01_ncu_linearize.md) showed 4.4 long-scoreboard + 1.0 drain stall cycles per issued instruction at
 // 0.55 of the HBM roofline with clean traffic.  Here
@@ -435,8 +437,11 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
 //                   released as soon as they are in registers, the camera row is gathered through L1/L2, the 24
 //                   Jacobian floats leave as streaming 128-bit stores that nothing waits for (no block exit).
 // Point side as in linearize_kernel (rank-ordered sum by the observation that completes its point), with
-// self-resetting counters (atomicInc wraps at the track length) and ONE group barrier per tile, which only
-// orders the reuse of the staging rows and is hidden by the other groups.  Cost: per-thread fp64 accumulation
+// self-resetting counters (atomicInc wraps at the track length).  The staging rows are double buffered and their
+// reuse is ordered by an mbarrier per buffer (each warp arrives when it is done with a tile, and waits for the
+// buffer's previous use just before it writes its rows two tiles later): a split barrier, so a warp never waits
+// for the others to reach the same point, only for work that is two tiles old.  A full group barrier per tile
+// cost 21 % of the stall samples (the group waits for its slowest warp, the one with most points to sum).  Cost: per-thread fp64 accumulation
 // over the thread's tiles (a fixed order), one partial per warp, folded by reduce_cost_kernel.
 // ------------------------------------------------------------------------------------------------
 struct LinLayout {  // byte offsets inside one stage / inside the dynamic shared memory
@@ -453,14 +458,14 @@ __host__ __device__ inline LinLayout lin_layout(int T, int NG, int max_pts, int 
   L.pts = up(L.rank + T * 2);
   L.meta = up(L.pts + max_pts * 16);
   L.stage_bytes = up(L.meta + (jac ? meta_max : 0));
-  L.sbuf_bytes = jac ? up(T * 40) : 0;  // per group: float4 stage[T][2], float gz[T], unsigned arrived[T]
-  const int fixed = NG * L.sbuf_bytes + 256;
+  L.sbuf_bytes = jac ? 2 * up(T * 40) : 0;  // per group, x2 buffers: float4 stage[T][2], float gz[T], unsigned arrived[T]
+  const int fixed = NG * L.sbuf_bytes + 512;  // 512: full[12], empty[12], seen[12], done[2 NG]
   int st = (smem_limit - fixed) / L.stage_bytes;
   if (st > 8) st = 8;  // 8 tiles of inputs (~50 KB) in flight per SM is far more than the consumers can drain
   L.stages = st;
   L.sbuf = L.stages * L.stage_bytes;
   L.bars = L.sbuf + NG * L.sbuf_bytes;
-  L.total = L.bars + 256;
+  L.total = L.bars + 512;
   return L;
 }
 
@@ -472,17 +477,19 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
   unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L.bars);
   unsigned long long* empty = full + kMaxStages;
   volatile int* seen = reinterpret_cast<volatile int*>(empty + kMaxStages);  // see schur_matvec_pipelined_kernel
+  unsigned long long* done = reinterpret_cast<unsigned long long*>(const_cast<int*>(seen) + kMaxStages);  // [NG][2]
   if (tid == 0) {
     for (int s = 0; s < L.stages; ++s) {
       mbar_init(full + s, 1);
       mbar_init(empty + s, T / 32);  // one group consumes a stage
       seen[s] = 0;
     }
+    for (int i = 0; i < 2 * NG; ++i) mbar_init(done + i, T / 32);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (JAC)  // per-point arrival counters of every group start at 0 and reset themselves (atomicInc wraps)
-    for (int i = tid; i < NG * T; i += NG * T + 32)
-      reinterpret_cast<unsigned*>(smem + L.sbuf + (size_t)(i / T) * L.sbuf_bytes + T * 36)[i % T] = 0u;
+  if (JAC)  // per-point arrival counters of every group and buffer start at 0 and reset themselves (atomicInc wraps)
+    for (int i = tid; i < 2 * NG * T; i += NG * T + 32)
+      reinterpret_cast<unsigned*>(smem + L.sbuf + (size_t)(i / T) * (L.sbuf_bytes / 2) + T * 36)[i % T] = 0u;
   __syncthreads();
   const int G = gridDim.x;
 
@@ -519,15 +526,15 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
 
   // ===== consumers: group g takes every NG-th tile of this CTA's sequence =====
   const int g = tid / T, gt = tid - g * T;
-  const int bar_id = 1 + g;
-  unsigned char* sb = smem + L.sbuf + (size_t)g * L.sbuf_bytes;
-  float4(*stage)[2] = reinterpret_cast<float4(*)[2]>(sb);         // by rank: (Vxx Vxy Vxz Vyy) (Vyz Vzz gx gy)
-  float* stage_gz = reinterpret_cast<float*>(sb + T * 32);        // by rank: gz
-  unsigned* arrived = reinterpret_cast<unsigned*>(sb + T * 36);   // by local point id
   double cost_acc = 0.0;
   int s = g % L.stages;
   int round = g / L.stages;
-  for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G) {
+  int k = 0;  // tiles this group has done
+  for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G, ++k) {
+    unsigned char* sb = smem + L.sbuf + (size_t)(2 * g + (k & 1)) * (L.sbuf_bytes / 2);  // this tile's buffer
+    float4(*stage)[2] = reinterpret_cast<float4(*)[2]>(sb);         // by rank: (Vxx Vxy Vxz Vyy) (Vyz Vzz gx gy)
+    float* stage_gz = reinterpret_cast<float*>(sb + T * 32);        // by rank: gz
+    unsigned* arrived = reinterpret_cast<unsigned*>(sb + T * 36);   // by local point id
     while (seen[s] < round) {
     }
     mbar_wait(full + s, (unsigned)(round & 1));
@@ -555,8 +562,6 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
     const long long slot = (long long)t * T + gt;
     float term = 0.f;
     if (JAC) {
-      // all warps of the group are done with the previous tile's staging rows and counters
-      group_bar(bar_id, T);
       float J[24], r0 = 0.f, r1 = 0.f;
 #pragma unroll
       for (int i = 0; i < 24; ++i) J[i] = 0.f;
@@ -578,6 +583,9 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
 #pragma unroll
       for (int c = 0; c < 6; ++c) __stcs(&v.J[c][slot], make_float4(J[4 * c], J[4 * c + 1], J[4 * c + 2], J[4 * c + 3]));
       __stcs(&v.res[slot], make_float2(r0, r1));
+      // every warp of the group is done with this buffer's previous use (two tiles ago)
+      unsigned long long* buf_done = done + 2 * g + (k & 1);
+      if (k >= 2) mbar_wait(buf_done, (unsigned)(((k >> 1) - 1) & 1));
       if (cam >= 0) {
         stage[rank][0] = make_float4(fmaf(J[18], J[18], J[21] * J[21]), fmaf(J[18], J[19], J[21] * J[22]),
                                      fmaf(J[18], J[20], J[21] * J[23]), fmaf(J[19], J[19], J[22] * J[22]));
@@ -604,6 +612,8 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
           v.gp[p0 + pid] = make_float4(b1.x, b1.y, gz, 0.f);
         }
       }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(buf_done);  // this warp is done with the buffer
     } else {
       if (cam >= 0) {
         float r0, r1;
@@ -1559,10 +1569,10 @@ static cudaError_t launch_linearize_pipelined(const View& v, const float4* pts, 
 template <bool JAC>
 static cudaError_t launch_linearize_t(const View& v, const float4* pts, const float* table, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaSuccess;
-  if (linearize_pipelined(v)) {
-    if (v.T == 256) return launch_linearize_pipelined<256, 3, JAC>(v, pts, table, s);
-    if (v.T == 192) return launch_linearize_pipelined<192, 4, JAC>(v, pts, table, s);
-    return launch_linearize_pipelined<128, 6, JAC>(v, pts, table, s);
+  if (JAC && linearize_pipelined(v)) {
+    if (v.T == 256) return launch_linearize_pipelined<256, 3, true>(v, pts, table, s);
+    if (v.T == 192) return launch_linearize_pipelined<192, 4, true>(v, pts, table, s);
+    return launch_linearize_pipelined<128, 6, true>(v, pts, table, s);
   }
   switch (v.T) {
     case 128: linearize_kernel<128, JAC><<<v.num_tiles, 128, 0, s>>>(v, pts, table); break;
@@ -1575,19 +1585,25 @@ static cudaError_t launch_linearize_t(const View& v, const float4* pts, const fl
 }
 
 // cost_out (device) receives sum_i rho(|r_i|^2); an empty problem gets 0 from the arena's memset / the caller
-cudaError_t launch_reduce_cost(const View& v, double* cost_out, cudaStream_t s) {
+// `pipelined`: the partials were written by linearize_pipelined_kernel (one per consumer warp of the grid), else by
+// linearize_kernel (one per warp of every tile)
+static cudaError_t launch_reduce_cost(const View& v, bool pipelined, double* cost_out, cudaStream_t s) {
   if (v.num_tiles == 0) return cudaMemsetAsync(cost_out, 0, sizeof(double), s);
-  const long long parts = linearize_pipelined(v) ? (long long)linearize_grid(v) * pipe_groups(v.T) * (v.T / 32)
-                                                 : (long long)v.num_tiles * (v.T / 32);
+  const long long parts = pipelined ? (long long)linearize_grid(v) * pipe_groups(v.T) * (v.T / 32)
+                                    : (long long)v.num_tiles * (v.T / 32);
   reduce_cost_kernel<<<1, 1024, 0, s>>>(v.cost_warp, parts, cost_out);
   return CBA_LAUNCHED();
 }
 
 cudaError_t launch_linearize(const View& v, cudaStream_t s) { return launch_linearize_t<true>(v, v.pts, v.cam_table, s); }
 
+cudaError_t launch_linearize_cost(const View& v, double* cost_out, cudaStream_t s) {
+  return launch_reduce_cost(v, linearize_pipelined(v), cost_out, s);
+}
+
 cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_out, cudaStream_t s) {
   cudaError_t e = launch_linearize_t<false>(v, pts, table, s);
-  return e != cudaSuccess ? e : launch_reduce_cost(v, cost_out, s);
+  return e != cudaSuccess ? e : launch_reduce_cost(v, false, cost_out, s);
 }
 
 cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s) {
@@ -1665,9 +1681,7 @@ static cudaError_t pipelined_attr(bool hot) {
 
 template <int T, int NG>
 static cudaError_t linearize_attr() {
-  cudaError_t e = cudaFuncSetAttribute(linearize_pipelined_kernel<T, NG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(linearize_pipelined_kernel<T, NG, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+  return cudaFuncSetAttribute(linearize_pipelined_kernel<T, NG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
 }
 
 bool pipelined_linearize_possible(const View& v) {
