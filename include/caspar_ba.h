@@ -115,6 +115,16 @@ int caspar_ba_linearize(caspar_ba_t* h, void* cuda_stream, double* cost_out);
 int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, void* cuda_stream,
                         caspar_ba_pcg_info* info);
 
+/* PAPER.md:163 ("does not rely on Schur decomposition and instead solves the linear normal equations directly"),
+ * :167-169 (PCG with normal residual: J and J^T applied separately, matrix-free) -- the paper's own linear solve
+ * (N1): preconditioned CG on the FULL system (J^T J + lambda D) delta = -g over cameras and points, block
+ * Jacobi with one block per node (U'_j, V'_k), x0 = 0, stop when |r_k| <= rel_tol |g| or after max_iter passes over
+ * the Jacobians.  Same state machine, info and errors as caspar_ba_pcg_solve; leaves delta in the arena. */
+int caspar_ba_pcgnr_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, void* cuda_stream,
+                          caspar_ba_pcg_info* info);
+/* Linear solver of caspar_ba_lm_step / caspar_ba_solve: 0 = Schur PCG (north_star, default), 1 = caspar_ba_pcgnr_solve. */
+int caspar_ba_set_linear_solver(caspar_ba_t* h, int32_t mode);
+
 /* PAPER.md:163 (Levenberg-Marquardt, quality-based damping after Madsen et al.: the gain ratio decides) --
  * steps S1-S10: linearize if the cache is stale, pcg_solve, evaluate the trial point x + delta, gain ratio,
  * then commit (parameters updated in place, cache stale) or discard (cache stays valid).
@@ -135,6 +145,13 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
  * lambdas[iterations] (HOST, nullable) receive each step's record and the lambda it was solved with. */
 int caspar_ba_solve(caspar_ba_t* h, int32_t iterations, float lambda0, float rel_tol, int32_t max_iter,
                     void* cuda_stream, caspar_ba_step_info* infos, float* lambdas);
+
+/* PAPER.md:163 ("block Jacobi preconditioner ... one block per node") -- preconditioner of the Schur PCG:
+ * 0 = blockdiag(U'_j), the damped camera blocks (default; C9); 1 = the diagonal 9x9 blocks of the Schur
+ * complement itself, S_jj = U'_j - sum_{i in j} W_i V'^-1 W_i^T ("Schur-Jacobi", N4): one more
+ * camera-ordered pass over the stored Jacobians per lambda, 5-25 % fewer PCG iterations.  Takes effect at the
+ * next solve.  Errors: EINVAL. */
+int caspar_ba_set_preconditioner(caspar_ba_t* h, int32_t mode);
 
 /* PAPER.md:194-203 (residual only), :220 (fp32 summation is the paper's stated accuracy loss: the sum is fp64 here) --
  * step S9 without the update: F at the caller's current parameters.  cost_out: HOST, required. */
@@ -159,7 +176,8 @@ enum {
   CASPAR_BA_V = 4,         /* [Np][3][3]                                         */
   CASPAR_BA_G = 5,         /* [9 Nc + 3 Np]                                      */
   CASPAR_BA_SCHUR_RHS = 6, /* [9 Nc]        (after pcg_solve)                    */
-  CASPAR_BA_DELTA = 7      /* [9 Nc + 3 Np] (after pcg_solve)                    */
+  CASPAR_BA_DELTA = 7,     /* [9 Nc + 3 Np] (after pcg_solve)                    */
+  CASPAR_BA_PRECONDITIONER = 8 /* [Nc][9][9] the blocks the preconditioner inverts (after pcg_solve / schur_matvec) */
 };
 /* device_dst: DEVICE double array with exactly `count` elements of the shape above. */
 int caspar_ba_export(caspar_ba_t* h, int32_t what, double* device_dst, size_t count, void* cuda_stream);

@@ -17,14 +17,14 @@ import torch
 from . import build as _build
 
 OK, EINVAL, ECUDA, ENOMEM, ENUMERIC, ESTATE = 0, -1, -2, -3, -4, -5
-RESIDUALS, JC, JP, U, V, G, SCHUR_RHS, DELTA = range(8)
+RESIDUALS, JC, JP, U, V, G, SCHUR_RHS, DELTA, PRECONDITIONER = range(9)
 
 EXPORTED_SYMBOLS = [
     "caspar_ba_create", "caspar_ba_linearize", "caspar_ba_pcg_solve", "caspar_ba_lm_step", "caspar_ba_solve",
     "caspar_ba_cost", "caspar_ba_destroy", "caspar_ba_set_parameters_host", "caspar_ba_get_parameters_host",
     "caspar_ba_export", "caspar_ba_schur_matvec", "caspar_ba_get_stats", "caspar_ba_set_profiling",
     "caspar_ba_last_error", "caspar_ba_layout_create", "caspar_ba_layout_get_info", "caspar_ba_layout_copy",
-    "caspar_ba_layout_destroy",
+    "caspar_ba_layout_destroy", "caspar_ba_set_preconditioner", "caspar_ba_pcgnr_solve", "caspar_ba_set_linear_solver",
 ]
 
 
@@ -125,6 +125,9 @@ def load_library() -> C.CDLL:
     L.caspar_ba_layout_copy.argtypes = [vp, C.c_int32, vp, C.c_size_t]
     L.caspar_ba_layout_destroy.argtypes = [vp]
     L.caspar_ba_layout_destroy.restype = None
+    L.caspar_ba_set_preconditioner.argtypes = [vp, C.c_int32]
+    L.caspar_ba_set_linear_solver.argtypes = [vp, C.c_int32]
+    L.caspar_ba_pcgnr_solve.argtypes = [vp, C.c_float, C.c_float, C.c_int32, vp, C.POINTER(PcgInfo)]
     _lib = L
     return L
 
@@ -241,6 +244,15 @@ class CasparBA:
                                                   C.byref(info)), "pcg_solve")
         return info
 
+    def pcgnr_solve(self, lam: float, rel_tol: float, max_iter: int, stream=None) -> PcgInfo:
+        info = PcgInfo()
+        self._check(self._lib.caspar_ba_pcgnr_solve(self._h, lam, rel_tol, max_iter, _stream_ptr(stream, self.device),
+                                                    C.byref(info)), "pcgnr_solve")
+        return info
+
+    def set_linear_solver(self, mode: int):
+        self._check(self._lib.caspar_ba_set_linear_solver(self._h, int(mode)), "set_linear_solver")
+
     def lm_step(self, lam: float, rel_tol: float, max_iter: int, accept_mode: int = 0, stream=None) -> Step:
         info = StepInfo()
         self._check(self._lib.caspar_ba_lm_step(self._h, lam, rel_tol, max_iter, accept_mode, _stream_ptr(stream, self.device),
@@ -268,14 +280,16 @@ class CasparBA:
     def export(self, what: int, stream=None) -> np.ndarray:
         nc, np_, n = self.nc, self.np_, self.n
         shape = {RESIDUALS: (n, 2), JC: (n, 2, 9), JP: (n, 2, 3), U: (nc, 9, 9), V: (np_, 3, 3),
-                 G: (9 * nc + 3 * np_,), SCHUR_RHS: (9 * nc,), DELTA: (9 * nc + 3 * np_,)}[what]
+                 G: (9 * nc + 3 * np_,), SCHUR_RHS: (9 * nc,), DELTA: (9 * nc + 3 * np_,),
+                 PRECONDITIONER: (nc, 9, 9)}[what]
         return self.export_device(what, stream).cpu().numpy()
 
     def export_device(self, what: int, stream=None) -> torch.Tensor:
         """The same export left on the device (fp64, caller's order): full-size tests sample it there."""
         nc, np_, n = self.nc, self.np_, self.n
         shape = {RESIDUALS: (n, 2), JC: (n, 2, 9), JP: (n, 2, 3), U: (nc, 9, 9), V: (np_, 3, 3),
-                 G: (9 * nc + 3 * np_,), SCHUR_RHS: (9 * nc,), DELTA: (9 * nc + 3 * np_,)}[what]
+                 G: (9 * nc + 3 * np_,), SCHUR_RHS: (9 * nc,), DELTA: (9 * nc + 3 * np_,),
+                 PRECONDITIONER: (nc, 9, 9)}[what]
         count = int(np.prod(shape))
         out = torch.zeros(max(count, 1), dtype=torch.float64, device=self.device)
         self._check(self._lib.caspar_ba_export(self._h, what, out.data_ptr(), count, _stream_ptr(stream, self.device)),
@@ -298,6 +312,9 @@ class CasparBA:
         st = Stats()
         self._check(self._lib.caspar_ba_get_stats(self._h, C.byref(st)), "get_stats")
         return st
+
+    def set_preconditioner(self, mode: int):
+        self._check(self._lib.caspar_ba_set_preconditioner(self._h, int(mode)), "set_preconditioner")
 
     def set_profiling(self, enable: bool):
         self._check(self._lib.caspar_ba_set_profiling(self._h, int(enable)), "set_profiling")

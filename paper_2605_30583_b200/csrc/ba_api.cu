@@ -28,6 +28,9 @@ struct caspar_ba {
   bool have_delta = false;
   double prepared_lambda = -1.0;
   bool prepared = false;
+  int prepared_preconditioner = 0;
+  int linear_solver = 0;   // of lm_step / solve: 0 = Schur PCG, 1 = full-system PCGNR (caspar_ba_set_linear_solver)
+  int preconditioner = 0;  // of the Schur PCG: 0 = blockdiag(U'_j), 1 = diagonal blocks of S (caspar_ba_set_preconditioner)
   double cost = 0.0;  // F at the cached linearization
   std::string err;
   long long launches = 0;
@@ -147,11 +150,17 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.gp = c.take<float4>(NP);
   v.Vinv = c.take<float4>(2 * NP);
   v.dp = c.take<float4>(NP);
+  v.xp = c.take<double>(3 * NP);
+  v.rp = c.take<double>(3 * NP);
+  v.pp32 = c.take<float4>(NP);
+  v.qp = c.take<float4>(NP);
   v.cams_trial = c.take<float>(9 * NC);
   v.cam_table = c.take<float>(kCamTableFloats * NC);
   v.cam_table_trial = c.take<float>(kCamTableFloats * NC);
   v.Ug = c.take<double>(kUg * NC);
   v.Minv = c.take<double>(81 * NC);
+  v.Pblk = c.take<double>(81 * NC);
+  v.Sdiag = c.take<double>(45 * NC);
   v.lamD = c.take<double>(9 * NC);
   v.b = c.take<double>(9 * NC);
   v.x = c.take<double>(9 * NC);
@@ -249,12 +258,13 @@ int do_linearize(caspar_ba* h, cudaStream_t s) {
   return 0;
 }
 
-int do_prepare(caspar_ba* h, double lambda, cudaStream_t s) {
-  if (h->prepared && h->prepared_lambda == lambda) return 0;
-  CK(launch_prepare_blocks(h->v, lambda, s));
+int do_prepare(caspar_ba* h, double lambda, int preconditioner, cudaStream_t s) {
+  if (h->prepared && h->prepared_lambda == lambda && h->prepared_preconditioner == preconditioner) return 0;
+  CK(launch_prepare_blocks(h->v, lambda, preconditioner, s));
   account(h);
   h->prepared = true;
   h->prepared_lambda = lambda;
+  h->prepared_preconditioner = preconditioner;
   return 0;
 }
 
@@ -283,7 +293,7 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
   View& v = h->v;
   h->prepared = false;  // the right-hand side b is rebuilt by prepare (it starts from -g_c)
   CK(cudaMemsetAsync(&v.step->jd2, 0, 2 * sizeof(double) + 2 * sizeof(int), s));  // jd2, dg, bad_block
-  int rc = do_prepare(h, lambda, s);
+  int rc = do_prepare(h, lambda, h->preconditioner, s);
   if (rc) return rc;
   CK(cudaMemsetAsync(v.pcg, 0, sizeof(PcgScalars), s));
   CK(launch_schur_rhs(v, s));
@@ -326,6 +336,45 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
   CK(launch_backsub(v, s));
   account(h);
   h->have_delta = true;
+  return 0;
+}
+
+// N1: enqueue the full-system PCG with normal residual (no Schur elimination).  Same device-side scalars, flags and
+// polling as do_pcg; every iteration is one pass over the Jacobians plus four vector kernels.
+int do_pcgnr(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream_t s) {
+  View& v = h->v;
+  h->prepared = false;  // b is rebuilt by prepare (it starts from -g_c)
+  CK(cudaMemsetAsync(&v.step->jd2, 0, 2 * sizeof(double) + 2 * sizeof(int), s));  // jd2, dg, bad_block
+  int rc = do_prepare(h, lambda, 0, s);  // one block per node: U'_j and V'_k
+  if (rc) return rc;
+  CK(cudaMemsetAsync(v.pcg, 0, sizeof(PcgScalars), s));
+  CK(launch_pcgnr_init(v, lambda, rel_tol * rel_tol, s));
+  const int chunk = kPcgChunk;
+  int polled = 0;
+  bool stop = false;
+  for (int it = 0; it < max_iter && !stop; ++it) {
+    {
+      Timed t(h, &h->ev_mv, s);
+      CK(launch_full_matvec(v, s));
+    }
+    CK(launch_pcgnr_update(v, lambda, s));
+    if (rel_tol > 0.0 && (it + 1) % chunk == 0 && it + 1 < max_iter) {
+      const int slot = polled & 1;
+      if (polled >= 2) {
+        CK(cudaEventSynchronize(h->poll_ev[slot]));
+        if (h->h_flags[slot]) stop = true;
+      }
+      if (!stop) {
+        CK(cudaMemcpyAsync(&h->h_flags[slot], &v.pcg->done, sizeof(int), cudaMemcpyDeviceToHost, s));
+        CK(cudaEventRecord(h->poll_ev[slot], s));
+        ++polled;
+      }
+    }
+  }
+  CK(launch_pcgnr_finish(v, s));
+  account(h);
+  h->have_delta = true;
+  h->prepared = false;  // v.b holds -g_c, not a Schur right-hand side
   return 0;
 }
 
@@ -562,6 +611,26 @@ int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max
   return check_numeric(h);
 }
 
+int caspar_ba_pcgnr_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, void* cuda_stream,
+                          caspar_ba_pcg_info* info) {
+  if (!h || max_iter < 0 || !(lambda >= 0.f) || !(rel_tol >= 0.f)) return CASPAR_BA_EINVAL;
+  if (!h->linearized) return fail(h, CASPAR_BA_ESTATE, "pcgnr_solve before linearize");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceGuard on_device(h->device);
+  int rc = do_pcgnr(h, (double)lambda, (double)rel_tol, max_iter, s);
+  if (rc) return rc;
+  rc = sync_step_scalars(h, s);
+  if (rc) return rc;
+  if (info) fill_pcg_info(h, info);
+  return check_numeric(h);
+}
+
+int caspar_ba_set_linear_solver(caspar_ba_t* h, int32_t mode) {
+  if (!h || (mode != 0 && mode != 1)) return CASPAR_BA_EINVAL;
+  h->linear_solver = mode;
+  return CASPAR_BA_OK;
+}
+
 int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, int32_t accept_mode,
                       void* cuda_stream, caspar_ba_step_info* info) {
   if (!h || !info || max_iter < 0 || accept_mode < 0 || accept_mode > 2 || !(lambda >= 0.f) || !(rel_tol >= 0.f))
@@ -576,7 +645,8 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
     rc = do_linearize(h, s);
     if (rc) return rc;
   }
-  rc = do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
+  rc = h->linear_solver == 1 ? do_pcgnr(h, (double)lambda, (double)rel_tol, max_iter, s)
+                             : do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
   if (rc) return rc;
   // trial point and its cost (S9)
   CK(launch_trial_update(v, s));
@@ -691,11 +761,13 @@ int caspar_ba_export(caspar_ba_t* h, int32_t what, double* device_dst, size_t co
     case CASPAR_BA_V: need = 9 * np; break;
     case CASPAR_BA_G: case CASPAR_BA_DELTA: need = 9 * nc + 3 * np; break;
     case CASPAR_BA_SCHUR_RHS: need = 9 * nc; break;
+    case CASPAR_BA_PRECONDITIONER: need = 81 * nc; break;
     default: return fail(h, CASPAR_BA_EINVAL, "unknown export id");
   }
   if (count != need) return fail(h, CASPAR_BA_EINVAL, "export: wrong element count");
   const bool solve_product = what == CASPAR_BA_SCHUR_RHS || what == CASPAR_BA_DELTA;
-  if (solve_product ? !h->have_delta : !h->linearized) return fail(h, CASPAR_BA_ESTATE, "export: nothing cached");
+  if (what == CASPAR_BA_PRECONDITIONER ? !h->prepared : (solve_product ? !h->have_delta : !h->linearized))
+    return fail(h, CASPAR_BA_ESTATE, "export: nothing cached");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   DeviceGuard on_device(h->device);
   CK(launch_export(h->v, what, device_dst, s));
@@ -709,7 +781,7 @@ int caspar_ba_schur_matvec(caspar_ba_t* h, float lambda, const double* p_dev, do
   if (!h->linearized) return fail(h, CASPAR_BA_ESTATE, "schur_matvec before linearize");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   DeviceGuard on_device(h->device);
-  int rc = do_prepare(h, (double)lambda, s);
+  int rc = do_prepare(h, (double)lambda, h->preconditioner, s);
   if (rc) return rc;
   CK(cudaMemsetAsync(h->v.pcg, 0, sizeof(PcgScalars), s));
   {
@@ -721,6 +793,12 @@ int caspar_ba_schur_matvec(caspar_ba_t* h, float lambda, const double* p_dev, do
   rc = sync_step_scalars(h, s);
   if (rc) return rc;
   return check_numeric(h);
+}
+
+int caspar_ba_set_preconditioner(caspar_ba_t* h, int32_t mode) {
+  if (!h || (mode != 0 && mode != 1)) return CASPAR_BA_EINVAL;
+  h->preconditioner = mode;  // do_prepare rebuilds the blocks when the mode they were built for differs
+  return CASPAR_BA_OK;
 }
 
 int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {

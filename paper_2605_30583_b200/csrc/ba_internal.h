@@ -110,12 +110,19 @@ struct View {
   float4* gp;             // g_p,k (xyz, w unused)
   float4* Vinv;           // V'^-1, two float4 per point: (xx xy xz yy) (yz zz 0 0) — 32 B, bulk-copy aligned
   float4* dp;             // delta_p,k
+  // full-system PCG (N1): point part of the state
+  double* xp;             // [3 np] x_p
+  double* rp;             // [3 np] r_p
+  float4* pp32;           // [np] search direction * pscale
+  float4* qp;             // [np] (J^T J p)_p of the current matvec, without the lambda D p term
   // per camera
   float* cams_trial;      // [nc][9]
   float* cam_table;       // [nc][kCamTableFloats]
   float* cam_table_trial;
   double* Ug;             // [nc][54]
   double* Minv;           // [nc][81]
+  double* Pblk;           // [nc][81] the blocks Minv inverts: U'_j or S_jj (test export)
+  double* Sdiag;          // [nc][45] sum_{i in j} J_c^T (I - B_i) J_c: the Schur-Jacobi blocks without lambda D_j
   double* lamD;           // [9 nc]
   double* b;              // [9 nc] Schur right-hand side
   double* x;              // [9 nc] delta_c
@@ -176,7 +183,7 @@ cudaError_t launch_linearize(const View& v, cudaStream_t s);
 cudaError_t launch_linearize_cost(const View& v, double* cost_out, cudaStream_t s);  // folds launch_linearize's partials
 cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_out, cudaStream_t s);
 cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s);
-cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s);
+cudaError_t launch_prepare_blocks(const View& v, double lambda, int preconditioner, cudaStream_t s);
 cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);
 cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s);
 cudaError_t launch_schur_matvec(const View& v, cudaStream_t s);
@@ -187,6 +194,10 @@ bool pipelined_matvec_available(const View& v);  // = v.pipeline
 int pipeline_stages(const View& v);
 cudaError_t launch_pcg_update(const View& v, cudaStream_t s);  // two kernels
 cudaError_t launch_backsub(const View& v, cudaStream_t s);
+cudaError_t launch_full_matvec(const View& v, cudaStream_t s);
+cudaError_t launch_pcgnr_init(const View& v, double lambda, double tol2, cudaStream_t s);
+cudaError_t launch_pcgnr_update(const View& v, double lambda, cudaStream_t s);  // four kernels
+cudaError_t launch_pcgnr_finish(const View& v, cudaStream_t s);
 cudaError_t launch_trial_update(const View& v, cudaStream_t s);
 cudaError_t launch_commit(const View& v, cudaStream_t s);
 cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s);

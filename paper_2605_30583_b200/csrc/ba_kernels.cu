@@ -717,10 +717,96 @@ __global__ void __launch_bounds__(64) reduce_camera_chunks_kernel(View v) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// N4 Schur-Jacobi preconditioner ("one block per node"): the diagonal 9x9 blocks of
+// the Schur complement itself,
+//   S_jj = U'_j - sum_{i in j} W_i V'^-1_k(i) W_i^T = lambda D_j + sum_{i in j} J_c,i^T (I - B_i) J_c,i,
+//   B_i = J_p,i V'^-1_k(i) J_p,i^T  (2x2, 0 <= B_i <= I),
+// assembled as a sum of positive semi-definite terms (no cancellation against U'_j at small lambda).  The same
+// camera-ordered chunk pass as assemble_cameras_kernel, with a 2x2 weight per observation; one partial row per
+// chunk, added in chunk order by reduce_camera_chunks_kernel (bitwise reproducible).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) assemble_schur_diagonal_kernel(View v) {
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (w >= v.num_chunks) return;
+  const int b = v.chunk_begin[w], e = v.chunk_begin[w + 1];
+  float acc[45];
+#pragma unroll
+  for (int i = 0; i < 45; ++i) acc[i] = 0.f;
+  for (int i = b + lane; i < e; i += 32) {
+    const int s = v.cslot[i];
+    float J[24];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      const float4 x = v.J[c][s];
+      J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
+    }
+    const int tile = s / v.T;
+    const unsigned pid = v.T <= 256 ? (unsigned)(v.rankpid[s] >> 8) : (v.rankpid32[s] >> 16);
+    const long long k = (long long)v.tile_pt[tile] + pid;
+    const float4 vi = __ldg(v.Vinv + 2 * k);
+    const float4 vj = __ldg(v.Vinv + 2 * k + 1);
+    // y = V'^-1 J_p^T (3x2), B = J_p y
+    const float* a = J + 18;  // J_p row 0
+    const float* c = J + 21;  // J_p row 1
+    const float ya0 = fmaf(vi.x, a[0], fmaf(vi.y, a[1], vi.z * a[2])), ya1 = fmaf(vi.y, a[0], fmaf(vi.w, a[1], vj.x * a[2])),
+                ya2 = fmaf(vi.z, a[0], fmaf(vj.x, a[1], vj.y * a[2]));
+    const float yc0 = fmaf(vi.x, c[0], fmaf(vi.y, c[1], vi.z * c[2])), yc1 = fmaf(vi.y, c[0], fmaf(vi.w, c[1], vj.x * c[2])),
+                yc2 = fmaf(vi.z, c[0], fmaf(vj.x, c[1], vj.y * c[2]));
+    const float m00 = 1.0f - fmaf(a[0], ya0, fmaf(a[1], ya1, a[2] * ya2));
+    const float m01 = -fmaf(a[0], yc0, fmaf(a[1], yc1, a[2] * yc2));
+    const float m11 = 1.0f - fmaf(c[0], yc0, fmaf(c[1], yc1, c[2] * yc2));
+    float z0[9], z1[9];  // (I - B) J_c
+#pragma unroll
+    for (int q = 0; q < 9; ++q) {
+      z0[q] = fmaf(m00, J[q], m01 * J[9 + q]);
+      z1[q] = fmaf(m01, J[q], m11 * J[9 + q]);
+    }
+    int idx = 0;
+#pragma unroll
+    for (int p = 0; p < 9; ++p)
+#pragma unroll
+      for (int q = p; q < 9; ++q) {
+        acc[idx] = fmaf(J[p], z0[q], fmaf(J[9 + p], z1[q], acc[idx]));
+        ++idx;
+      }
+  }
+  double mine0 = 0.0, mine1 = 0.0;
+#pragma unroll
+  for (int i = 0; i < 45; ++i) {
+    const double tot = warp_sum((double)acc[i]);
+    if ((i & 31) == lane) {
+      if (i < 32) mine0 = tot; else mine1 = tot;
+    }
+  }
+  double* dst = v.Ug_part + (long long)kUg * w;  // the per-chunk rows are free again once U, g_c are reduced
+  dst[lane] = mine0;
+  if (lane + 32 < 45) dst[lane + 32] = mine1;
+}
+
+__global__ void __launch_bounds__(64) reduce_schur_diagonal_kernel(View v) {
+  const int j = blockIdx.x, e = threadIdx.x;
+  if (e >= 45) return;
+  const int c0 = v.cam_chunk_ptr[j], c1 = v.cam_chunk_ptr[j + 1];
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  const double* src = v.Ug_part + (long long)kUg * c0 + e;
+  int c = c0;
+  for (; c + 4 <= c1; c += 4, src += 4 * kUg) {
+    a0 += src[0];
+    a1 += src[kUg];
+    a2 += src[2 * kUg];
+    a3 += src[3 * kUg];
+  }
+  if (c < c1) a0 += src[0];
+  if (c + 1 < c1) a1 += src[kUg];
+  if (c + 2 < c1) a2 += src[2 * kUg];
+  v.Sdiag[45ll * j + e] = (a0 + a1) + (a2 + a3);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Damped blocks for one lambda: M^-1 = (U + lambda D_c)^-1 per camera (fp64 Cholesky), lambda D_c,
 // the initial Schur right-hand side -g_c; V'^-1 = (V + lambda D_p)^-1 per point (fp64, stored fp32).
 // ------------------------------------------------------------------------------------------------
-__global__ void prepare_cameras_kernel(View v, double lambda) {
+__global__ void prepare_cameras_kernel(View v, double lambda, int schur_diagonal) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= v.nc) return;
   const double* ug = v.Ug + (long long)kUg * j;
@@ -734,11 +820,27 @@ __global__ void prepare_cameras_kernel(View v, double lambda) {
         ++k;
       }
   }
+  double ld[9];
   for (int a = 0; a < 9; ++a) {
     const double d = v.damping_mode == 1 ? 1.0 : fmax(A[10 * a], (double)kDMin);
-    v.lamD[9ll * j + a] = lambda * d;
-    A[10 * a] += lambda * d;
+    ld[a] = lambda * d;
+    v.lamD[9ll * j + a] = ld[a];
     v.b[9ll * j + a] = -ug[45 + a];
+  }
+  if (schur_diagonal) {  // S_jj = lambda D_j + sum J_c^T (I - B) J_c
+    const double* sd = v.Sdiag + 45ll * j;
+    int k = 0;
+    for (int a = 0; a < 9; ++a)
+      for (int c = a; c < 9; ++c) {
+        A[9 * a + c] = sd[k];
+        A[9 * c + a] = sd[k];
+        ++k;
+      }
+  }
+  for (int a = 0; a < 9; ++a) A[10 * a] += ld[a];
+  {
+    double* blk = v.Pblk + 81ll * j;  // the block the preconditioner inverts (test export)
+    for (int i = 0; i < 81; ++i) blk[i] = A[i];
   }
   bool ok = true;
   for (int i = 0; i < 81; ++i) L[i] = 0.0;
@@ -1372,6 +1474,243 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v) {
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// N1: the paper's own linear solve, PCG with normal residual on the FULL camera + point system,
+// no Schur elimination (PAPER.md:163 "solves the linear normal equations directly", :167-169 "the Jacobian and its
+// transpose are applied separately").  One pass over the stored Jacobians per iteration, in tile order:
+//   u_i = J_c,i p_c,j(i) + J_p,i p_p,k(i)                       (J applied, per observation)
+//   q_c,j += sum_{i in j} J_c,i^T u_i,   q_p,k = sum_{i in k} J_p,i^T u_i      (J^T applied: "shared add" on both sides)
+// camera side exactly as the Schur pass (in-tile camera runs, one fp64 RED per run and component), point side
+// through the rank-ordered staging rows (a point lives in one tile: plain stores, no atomics).  The lambda D p terms
+// and p.q = sum |u_i|^2 + p.lambda D p are completed by the update kernels.  FINAL: the same pass on delta instead of
+// the search direction, for |J delta|^2 of the gain ratio (ignores / keeps the PCG scalars).
+// ------------------------------------------------------------------------------------------------
+template <int T, bool FINAL>
+__global__ void __launch_bounds__(T, blocks_per_sm(T)) full_matvec_kernel(View v) {
+  __shared__ float stage[9][T + 1];
+  __shared__ double red[32];
+  const int t = blockIdx.x, tid = threadIdx.x;
+  if (!FINAL) {
+    if (v.pcg->done) return;
+    if (t == 0 && tid == 0) {  // accumulators of the update that follows this matvec
+      const int nxt = (v.pcg->it_a + 1) & 1;
+      v.pcg->rz[nxt] = 0.0;
+      v.pcg->pDp[nxt] = 0.0;
+      v.pcg->rr = 0.0;
+    }
+  }
+  const long long slot = (long long)t * T + tid;
+  const int p0 = v.tile_pt[t], p1 = v.tile_pt[t + 1];
+  const int base = v.pt_ptr[p0];
+  const int cam = v.cam[slot];
+  const unsigned rank = v.rank[slot];
+  float J[24];
+#pragma unroll
+  for (int c = 0; c < 6; ++c) {
+    const float4 x = __ldcs(&v.J[c][slot]);
+    J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
+  }
+  // the direction's point part, broadcast to the point's rank range
+  for (int k = p0 + tid; k < p1; k += T) {
+    const float4 pp = v.pp32[k];
+    for (int r = v.pt_ptr[k] - base; r < v.pt_ptr[k + 1] - base; ++r) { stage[0][r] = pp.x; stage[1][r] = pp.y; stage[2][r] = pp.z; }
+  }
+  __syncthreads();
+  float u0 = 0.f, u1 = 0.f;
+  if (cam >= 0) {
+    const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
+    const float4 a = __ldg(pv), b = __ldg(pv + 1), c = __ldg(pv + 2);
+    const float pj[9] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x};
+#pragma unroll
+    for (int i = 0; i < 9; ++i) {
+      u0 = fmaf(J[i], pj[i], u0);
+      u1 = fmaf(J[9 + i], pj[i], u1);
+    }
+    const float x0 = stage[0][rank], x1 = stage[1][rank], x2 = stage[2][rank];
+    u0 += fmaf(J[18], x0, fmaf(J[19], x1, J[20] * x2));
+    u1 += fmaf(J[21], x0, fmaf(J[22], x1, J[23] * x2));
+    stage[0][rank] = fmaf(J[18], u0, J[21] * u1);  // J_p^T u, at the same rank this thread just read
+    stage[1][rank] = fmaf(J[19], u0, J[22] * u1);
+    stage[2][rank] = fmaf(J[20], u0, J[23] * u1);
+  }
+  const double dot_part = (double)u0 * (double)u0 + (double)u1 * (double)u1;
+  if (!FINAL) {
+    __syncthreads();
+    for (int k = p0 + tid; k < p1; k += T) {
+      float t0 = 0.f, t1 = 0.f, t2 = 0.f;
+      for (int r = v.pt_ptr[k] - base; r < v.pt_ptr[k + 1] - base; ++r) { t0 += stage[0][r]; t1 += stage[1][r]; t2 += stage[2][r]; }
+      v.qp[k] = make_float4(t0, t1, t2, 0.f);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 9; ++i) stage[i][tid] = cam >= 0 ? fmaf(J[i], u0, J[9 + i] * u1) : 0.f;
+    __syncthreads();
+    const int rb = v.run_begin[t], nruns = v.run_begin[t + 1] - rb - 1;
+    for (int w = tid; w < 9 * nruns; w += T) {
+      const int u = w / 9, a = w - 9 * u;
+      const int s1 = v.run_slot[rb + u + 1];
+      float acc = 0.f;
+      for (int s = v.run_slot[rb + u]; s < s1; ++s) acc += stage[a][s];
+      atomicAdd(v.q + 9ll * v.run_cam[rb + u] + a, (double)acc);
+    }
+  }
+  const double tot = block_sum(dot_part, red);
+  if (tid == 0) atomicAdd(FINAL ? &v.step->jd2 : &v.pcg->pq, tot);
+}
+
+// ---- point part of the PCGNR vector updates.  The camera part is the Schur PCG's own kernels (pcg_norm / pcg_init /
+// pcg_update_xr / pcg_update_p with b = -g_c and M = blockdiag(U'_j)); both parts add to the same device scalars and
+// take the same decisions from them, and the point kernels run BEFORE the camera kernels of the same phase because
+// those advance the iteration counters and the direction scale.  State per point: x, r in fp64; the direction only
+// as the fp32 copy handed to the matvec (p = pp32 / pscale, a power of two); z = V'^-1 r is recomputed, not stored.
+__device__ __forceinline__ void point_damping(const View& v, int k, double lambda, double (&ld)[3]) {
+  if (v.damping_mode == 1) {
+    ld[0] = ld[1] = ld[2] = lambda;
+  } else {
+    const float4 a = v.V0[k];
+    const float2 c = v.V1[k];
+    ld[0] = lambda * fmax((double)a.x, (double)kDMin);
+    ld[1] = lambda * fmax((double)a.w, (double)kDMin);
+    ld[2] = lambda * fmax((double)c.y, (double)kDMin);
+  }
+}
+
+__device__ __forceinline__ void apply_vinv(const View& v, int k, const double (&r)[3], double (&z)[3]) {
+  const float4 vi = v.Vinv[2ll * k];
+  const float4 vj = v.Vinv[2ll * k + 1];
+  z[0] = (double)vi.x * r[0] + (double)vi.y * r[1] + (double)vi.z * r[2];
+  z[1] = (double)vi.y * r[0] + (double)vi.w * r[1] + (double)vj.x * r[2];
+  z[2] = (double)vi.z * r[0] + (double)vj.x * r[1] + (double)vj.y * r[2];
+}
+
+__global__ void __launch_bounds__(256) pcgnr_norm_points_kernel(View v) {
+  __shared__ double red[32];
+  const int k = blockIdx.x * 256 + threadIdx.x;
+  double s = 0.0;
+  if (k < v.np_obs) {
+    const float4 g = v.gp[k];
+    s = (double)g.x * g.x + (double)g.y * g.y + (double)g.z * g.z;
+  }
+  s = block_sum(s, red);
+  if (threadIdx.x == 0) atomicAdd(&v.pcg->bnorm2, s);
+}
+
+__global__ void __launch_bounds__(256) pcgnr_init_points_kernel(View v, double lambda) {
+  __shared__ double red[32];
+  const int k = blockIdx.x * 256 + threadIdx.x;
+  const double scale = direction_scale(v.pcg->bnorm2);
+  double s_rz = 0.0, s_rr = 0.0, s_pd = 0.0;
+  if (k < v.np_obs) {
+    const float4 g = v.gp[k];
+    const double r[3] = {-(double)g.x, -(double)g.y, -(double)g.z};
+    double z[3], ld[3];
+    apply_vinv(v, k, r, z);
+    point_damping(v, k, lambda, ld);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      v.xp[3ll * k + a] = 0.0;
+      v.rp[3ll * k + a] = r[a];
+      s_rz += r[a] * z[a];
+      s_rr += r[a] * r[a];
+    }
+    // the direction as the matvec sees it; p.lambda D p from the rounded direction (what alpha is applied to)
+    const float4 pp = make_float4((float)(z[0] * scale), (float)(z[1] * scale), (float)(z[2] * scale), 0.f);
+    v.pp32[k] = pp;
+    const double inv = 1.0 / scale;
+    s_pd = ld[0] * (pp.x * inv) * (pp.x * inv) + ld[1] * (pp.y * inv) * (pp.y * inv) + ld[2] * (pp.z * inv) * (pp.z * inv);
+  }
+  s_rz = block_sum(s_rz, red);
+  s_rr = block_sum(s_rr, red);
+  s_pd = block_sum(s_pd, red);
+  if (threadIdx.x == 0) {
+    atomicAdd(&v.pcg->rz[0], s_rz);
+    atomicAdd(&v.pcg->rr, s_rr);
+    atomicAdd(&v.pcg->pDp[0], s_pd);
+  }
+}
+
+__global__ void __launch_bounds__(256) pcgnr_update_xr_points_kernel(View v, double lambda) {
+  __shared__ double red[32];
+  const PcgScalars* sc = v.pcg;
+  if (sc->done) return;
+  const int par = sc->it_a & 1;
+  const double unscale = 1.0 / sc->pscale;
+  const double denom = sc->pq * unscale * unscale + sc->pDp[par];
+  const double rz = sc->rz[par];
+  if (!(denom > 0.0) || !isfinite(denom) || !isfinite(rz)) return;  // the camera kernel records the breakdown
+  const double alpha = rz / denom;
+  const int k = blockIdx.x * 256 + threadIdx.x;
+  double s_rz = 0.0, s_rr = 0.0;
+  if (k < v.np_obs) {
+    const float4 pp = v.pp32[k], qq = v.qp[k];
+    double ld[3], r[3], z[3];
+    point_damping(v, k, lambda, ld);
+    const double p[3] = {pp.x * unscale, pp.y * unscale, pp.z * unscale};
+    const double q[3] = {qq.x * unscale + ld[0] * p[0], qq.y * unscale + ld[1] * p[1], qq.z * unscale + ld[2] * p[2]};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      v.xp[3ll * k + a] += alpha * p[a];
+      r[a] = v.rp[3ll * k + a] - alpha * q[a];
+      v.rp[3ll * k + a] = r[a];
+    }
+    apply_vinv(v, k, r, z);
+    s_rz = r[0] * z[0] + r[1] * z[1] + r[2] * z[2];
+    s_rr = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+  }
+  s_rz = block_sum(s_rz, red);
+  s_rr = block_sum(s_rr, red);
+  if (threadIdx.x == 0) {
+    atomicAdd(&v.pcg->rz[par ^ 1], s_rz);
+    atomicAdd(&v.pcg->rr, s_rr);
+  }
+}
+
+__global__ void __launch_bounds__(256) pcgnr_update_p_points_kernel(View v, double lambda) {
+  __shared__ double red[32];
+  const PcgScalars* sc = v.pcg;
+  if (sc->done) return;
+  const int par = sc->it_b & 1;
+  if (sc->rr <= sc->tol2 * sc->bnorm2) return;  // converged: the camera kernel records it
+  const double beta = sc->rz[par ^ 1] / sc->rz[par];
+  const double unscale = 1.0 / sc->pscale, scale = direction_scale(sc->rr);
+  const int k = blockIdx.x * 256 + threadIdx.x;
+  double s_pd = 0.0;
+  if (k < v.np_obs) {
+    const float4 pp = v.pp32[k];
+    const double r[3] = {v.rp[3ll * k], v.rp[3ll * k + 1], v.rp[3ll * k + 2]};
+    double z[3], ld[3];
+    apply_vinv(v, k, r, z);
+    point_damping(v, k, lambda, ld);
+    const float4 pn = make_float4((float)((z[0] + beta * (pp.x * unscale)) * scale), (float)((z[1] + beta * (pp.y * unscale)) * scale),
+                                  (float)((z[2] + beta * (pp.z * unscale)) * scale), 0.f);
+    v.pp32[k] = pn;
+    const double inv = 1.0 / scale;
+    s_pd = ld[0] * (pn.x * inv) * (pn.x * inv) + ld[1] * (pn.y * inv) * (pn.y * inv) + ld[2] * (pn.z * inv) * (pn.z * inv);
+  }
+  s_pd = block_sum(s_pd, red);
+  if (threadIdx.x == 0) atomicAdd(&v.pcg->pDp[par ^ 1], s_pd);
+}
+
+// delta_p = x_p (fp32 for the trial update and the export), its fp32 copy as the direction of the final J delta
+// pass, and delta_p . g_p; unobserved points get 0
+__global__ void __launch_bounds__(256) pcgnr_finish_points_kernel(View v) {
+  __shared__ double red[32];
+  const int k = blockIdx.x * 256 + threadIdx.x;
+  double s = 0.0;
+  if (k < v.np) {
+    float4 d = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (k < v.np_obs) {
+      d = make_float4((float)v.xp[3ll * k], (float)v.xp[3ll * k + 1], (float)v.xp[3ll * k + 2], 0.f);
+      const float4 g = v.gp[k];
+      s = (double)d.x * g.x + (double)d.y * g.y + (double)d.z * g.z;
+      v.pp32[k] = d;
+    }
+    v.dp[k] = d;
+  }
+  s = block_sum(s, red);
+  if (threadIdx.x == 0) atomicAdd(&v.step->dg, s);
+}
+
 // delta_c -> fp32 padded copy for the back-substitution pass; delta_c . g_c
 __global__ void __launch_bounds__(kPcgThreads) delta_c_kernel(View v) {
   __shared__ double red[32];
@@ -1506,6 +1845,9 @@ __global__ void export_kernel(View v, int what, double* __restrict__ dst) {
     case CASPAR_BA_SCHUR_RHS:
       if (i < 9ll * v.nc) dst[i] = v.b[i];
       return;
+    case CASPAR_BA_PRECONDITIONER:
+      if (i < 81ll * v.nc) dst[i] = v.Pblk[i];
+      return;
   }
 }
 
@@ -1616,14 +1958,26 @@ cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s) {
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_prepare_blocks(const View& v, double lambda, cudaStream_t s) {
+// preconditioner: 0 = blockdiag(U'_j) (C9), 1 = the diagonal blocks of S (N4; needs V'^-1 first, and one more
+// camera-ordered pass over the Jacobians)
+cudaError_t launch_prepare_blocks(const View& v, double lambda, int preconditioner, cudaStream_t s) {
   cudaError_t e = cudaSuccess;
-  if (v.nc > 0) {
-    prepare_cameras_kernel<<<grid_for(v.nc, 64), 64, 0, s>>>(v, lambda);
+  if (v.np_obs > 0) {
+    prepare_points_kernel<<<grid_for(v.np_obs, 256), 256, 0, s>>>(v, lambda);
     e = CBA_LAUNCHED();
   }
-  if (e == cudaSuccess && v.np_obs > 0) {
-    prepare_points_kernel<<<grid_for(v.np_obs, 256), 256, 0, s>>>(v, lambda);
+  if (e == cudaSuccess && preconditioner == 1 && v.nc > 0) {
+    if (v.num_chunks > 0) {
+      assemble_schur_diagonal_kernel<<<grid_for(32ll * v.num_chunks, 128), 128, 0, s>>>(v);
+      e = CBA_LAUNCHED();
+    }
+    if (e == cudaSuccess) {
+      reduce_schur_diagonal_kernel<<<v.nc, 64, 0, s>>>(v);
+      e = CBA_LAUNCHED();
+    }
+  }
+  if (e == cudaSuccess && v.nc > 0) {
+    prepare_cameras_kernel<<<grid_for(v.nc, 64), 64, 0, s>>>(v, lambda, preconditioner);
     e = CBA_LAUNCHED();
   }
   return e;
@@ -1748,6 +2102,74 @@ cudaError_t launch_backsub(const View& v, cudaStream_t s) {
   return launch_pass<BACKSUB>(v, s);
 }
 
+template <bool FINAL>
+static cudaError_t launch_full_pass(const View& v, cudaStream_t s) {
+  if (v.num_tiles == 0) return cudaSuccess;
+  switch (v.T) {
+    case 128: full_matvec_kernel<128, FINAL><<<v.num_tiles, 128, 0, s>>>(v); break;
+    case 192: full_matvec_kernel<192, FINAL><<<v.num_tiles, 192, 0, s>>>(v); break;
+    case 256: full_matvec_kernel<256, FINAL><<<v.num_tiles, 256, 0, s>>>(v); break;
+    case 512: full_matvec_kernel<512, FINAL><<<v.num_tiles, 512, 0, s>>>(v); break;
+    default: full_matvec_kernel<1024, FINAL><<<v.num_tiles, 1024, 0, s>>>(v); break;
+  }
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_full_matvec(const View& v, cudaStream_t s) { return launch_full_pass<false>(v, s); }
+
+// x0 = 0, r0 = -g, z0 = M^-1 r0, p0 = z0 on both parts (b = -g_c was set by the block preparation)
+cudaError_t launch_pcgnr_init(const View& v, double lambda, double tol2, cudaStream_t s) {
+  if (v.nc == 0) return cudaSuccess;
+  const unsigned gc = grid_for(9ll * v.nc, kPcgThreads), gp = grid_for(v.np_obs, 256);
+  pcg_norm_kernel<<<gc, kPcgThreads, 0, s>>>(v);
+  cudaError_t e = CBA_LAUNCHED();
+  if (e == cudaSuccess && v.np_obs > 0) {
+    pcgnr_norm_points_kernel<<<gp, 256, 0, s>>>(v);
+    e = CBA_LAUNCHED();
+  }
+  if (e == cudaSuccess && v.np_obs > 0) {
+    pcgnr_init_points_kernel<<<gp, 256, 0, s>>>(v, lambda);
+    e = CBA_LAUNCHED();
+  }
+  if (e != cudaSuccess) return e;
+  pcg_init_kernel<<<gc, kPcgThreads, 0, s>>>(v, tol2);
+  return CBA_LAUNCHED();
+}
+
+cudaError_t launch_pcgnr_update(const View& v, double lambda, cudaStream_t s) {
+  if (v.nc == 0) return cudaSuccess;
+  const unsigned gc = grid_for(9ll * v.nc, kPcgThreads), gp = grid_for(v.np_obs, 256);
+  cudaError_t e = cudaSuccess;
+  if (v.np_obs > 0) {
+    pcgnr_update_xr_points_kernel<<<gp, 256, 0, s>>>(v, lambda);
+    e = CBA_LAUNCHED();
+  }
+  if (e != cudaSuccess) return e;
+  pcg_update_xr_kernel<<<gc, kPcgThreads, 0, s>>>(v);
+  e = CBA_LAUNCHED();
+  if (e == cudaSuccess && v.np_obs > 0) {
+    pcgnr_update_p_points_kernel<<<gp, 256, 0, s>>>(v, lambda);
+    e = CBA_LAUNCHED();
+  }
+  if (e != cudaSuccess) return e;
+  pcg_update_p_kernel<<<gc, kPcgThreads, 0, s>>>(v);
+  return CBA_LAUNCHED();
+}
+
+// delta = x on both parts, delta . g, and |J delta|^2 from one more pass with delta as the direction
+cudaError_t launch_pcgnr_finish(const View& v, cudaStream_t s) {
+  cudaError_t e = cudaSuccess;
+  if (v.nc > 0) {
+    delta_c_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
+    e = CBA_LAUNCHED();
+  }
+  if (e == cudaSuccess && v.np > 0) {
+    pcgnr_finish_points_kernel<<<grid_for(v.np, 256), 256, 0, s>>>(v);
+    e = CBA_LAUNCHED();
+  }
+  return e != cudaSuccess ? e : launch_full_pass<true>(v, s);
+}
+
 cudaError_t launch_trial_update(const View& v, cudaStream_t s) {
   const long long n = 9ll * v.nc > v.np ? 9ll * v.nc : v.np;
   if (n == 0) return cudaSuccess;
@@ -1770,6 +2192,7 @@ cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s) 
     case CASPAR_BA_V: n = v.np; break;
     case CASPAR_BA_G: case CASPAR_BA_DELTA: n = 9ll * v.nc > v.np ? 9ll * v.nc : v.np; break;
     case CASPAR_BA_SCHUR_RHS: n = 9ll * v.nc; break;
+    case CASPAR_BA_PRECONDITIONER: n = 81ll * v.nc; break;
     default: return cudaErrorInvalidValue;
   }
   if (n == 0) return cudaSuccess;
