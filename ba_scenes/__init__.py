@@ -5,4 +5,4 @@ CUDA path (`paper_2605_30583_b200/`).  It holds no solver arithmetic: it draws
 cameras, points and visibility from a seeded `numpy` generator and synthesises
 pixel measurements with scipy's rotation routine.  See DESIGN.md "Input recipe".
 """
-from .generator import CONFIGS, Scene, make_scene, scene_summary  # noqa: F401
+from .generator import CONFIGS, FULL_OBSERVATIONS, Scene, make_scene, scene_summary  # noqa: F401

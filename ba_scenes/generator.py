@@ -56,6 +56,10 @@ CONFIGS: Dict[str, dict] = {
                    outlier_range=300.0),
 }
 
+# Observations each full config yields (after the grazing cull; pinned by tests/test_generator.py and by the full-size
+# GPU tests): lets a caller size a sample against the full workload without generating it.
+FULL_OBSERVATIONS = {"tiny": 5_990, "small": 129_449, "mid": 5_035_057, "large": 28_810_876, "skewed": 15_213_972}
+
 GRID_SPACING = 2.0
 GRID_HEIGHT = 10.0
 RING_RADIUS = 10.0

@@ -45,11 +45,15 @@ def hbm_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+TRAFFIC_FILE = os.path.join("profiles", "r02_traffic.csv")
+
+
 def ncu_traffic(kernel: str):
-    """dram bytes per launch of `kernel` from the committed ncu --set full summary (profiles/r01_traffic.csv), if any."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on the Large scene, from the committed
+    `ncu --set full` summary (a builder run under ncu, not measured in this run: `traffic_source` says so)."""
     import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
+        with open(os.path.join(ROOT, TRAFFIC_FILE)) as fh:
             for row in csv.DictReader(fh):
                 if row["kernel"] == kernel:
                     return float(row["dram_bytes_per_launch"])
@@ -115,11 +119,14 @@ def nielsen(lam: float, nu: float, step):
 # ---------------------------------------------------------------------------------------------------
 # reference arm: the fp64 oracle, as it stands, on the host cores
 # ---------------------------------------------------------------------------------------------------
-def time_oracle(workload: str, steps: int, warmup: int, full_observations: int):
-    """LM iterations/s of the oracle on a bounded sample of `workload`; returns (value scaled to the full
-    workload, description dict)."""
+def time_oracle(workload: str, steps: int, warmup: int):
+    """The oracle, as it stands, on the box's host cores, on a BOUNDED SAMPLE of `workload` (the same recipe shrunk:
+    the full 'large' scene needs ~30 s per LM iteration and 6 GB of fp64 Jacobians).  Returns a description dict
+    whose `sample_lm_iterations_per_s` is MEASURED and whose `value` is that rate scaled by the observation count to
+    the full workload (`extrapolated`: the oracle is O(observations) per matvec; PCG iteration counts are the
+    sample's own)."""
     import oracle
-    from ba_scenes import CONFIGS, make_scene
+    from ba_scenes import CONFIGS, FULL_OBSERVATIONS, make_scene
 
     scene = make_scene(workload, **SAMPLES[workload])
     cfg = CONFIGS[workload]
@@ -135,34 +142,54 @@ def time_oracle(workload: str, steps: int, warmup: int, full_observations: int):
             elapsed += dt
             matvecs += st.pcg_iterations
         lam, nu = nielsen(lam, nu, st)
-    n_s = scene.num_observations
+    n_s, n_full = scene.num_observations, FULL_OBSERVATIONS[workload]
     per_it_sample = steps / elapsed
-    scale = n_s / max(1, full_observations)
-    desc = {"kind": "oracle", "cores": oracle.num_threads(),
+    factor = n_s / n_full
+    return {"kind": "oracle", "cores": oracle.num_threads(), "unit": "LM iterations/s",
+            "value": per_it_sample * factor, "extrapolated": factor != 1.0, "extrapolation_factor": factor,
             "sample": (f"{workload} recipe shrunk to {scene.num_cameras} cameras / {scene.num_points} points / "
                        f"{n_s} observations; {steps} LM iterations (PCG cap {cfg['pcg_max_iter']}, tol "
-                       f"{cfg['pcg_rel_tol']:g}; {matvecs} matvecs) took {elapsed:.2f} s = {per_it_sample:.3f} it/s on the "
-                       f"sample, scaled by observations ({n_s}/{full_observations}) to the full workload"),
-            "sample_lm_iterations_per_s": per_it_sample, "sample_observations": n_s,
+                       f"{cfg['pcg_rel_tol']:g}; {matvecs} matvecs) took {elapsed:.2f} s = {per_it_sample:.3f} it/s MEASURED "
+                       f"on the sample; `value` scales it by observations ({n_s}/{n_full})"),
+            "sample_lm_iterations_per_s": per_it_sample, "sample_observations": n_s, "sample_seconds": elapsed,
             "sample_matvecs_per_s": matvecs / elapsed}
-    return per_it_sample * scale, desc
+
+
+def time_oracle_single_thread(workload: str):
+    """One LM iteration of the same sample with OMP_NUM_THREADS=1, in a child process (the thread count is fixed
+    when the OpenMP runtime starts)."""
+    code = ("import json,sys,time; sys.path.insert(0, %r); import bench, oracle; from ba_scenes import CONFIGS, make_scene;"
+            "w=%r; s=make_scene(w, **bench.SAMPLES[w]); c=CONFIGS[w]; o=oracle.OracleBA.from_scene(s);"
+            "t=time.perf_counter(); st=o.lm_step(bench.LAMBDA0, c['pcg_rel_tol'], c['pcg_max_iter'], 0);"
+            "print(json.dumps({'seconds': time.perf_counter()-t, 'matvecs': st.pcg_iterations, 'cores': oracle.num_threads()}))"
+            % (ROOT, workload))
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, OMP_NUM_THREADS="1"),
+                             capture_output=True, text=True, timeout=600, check=True).stdout
+        d = json.loads(out.strip().splitlines()[-1])
+        return {"cores": d["cores"], "sample_lm_iterations_per_s": 1.0 / d["seconds"], "matvecs": d["matvecs"],
+                "what": "first LM iteration of the same sample, OMP_NUM_THREADS=1"}
+    except Exception as exc:  # reported, never fatal for the bench line
+        return {"error": str(exc)[:200]}
 
 
 def run_reference(args):
+    """--impl reference: the oracle on the host cores.  `value` and `ms_per_step` are MEASURED on the bounded sample
+    (not scaled); cpu_baseline carries the same number scaled to the full workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from ba_scenes import CONFIGS
-    full_obs = {"large": 28_810_903, "mid": 5_035_057, "skewed": 15_213_972, "small": 129_449, "tiny": 5_990}[args.workload]
     t0 = time.perf_counter()
-    value, desc = time_oracle(args.workload, args.steps, args.warmup, full_obs)
+    desc = time_oracle(args.workload, args.steps, args.warmup)
     wall = time.perf_counter() - t0
-    desc["value"] = value
     cfg = CONFIGS[args.workload]
+    value = desc["sample_lm_iterations_per_s"]
     line = {"impl": "reference", "metric": "lm_iterations_per_s", "value": value, "unit": "LM iterations/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / value,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"configs[3]-style '{args.workload}' (seed {cfg['seed']}), bounded sample, scaled",
+            "config": {"workload": f"BOUNDED SAMPLE of BASELINE.json configs '{args.workload}' (seed {cfg['seed']}): "
+                                   f"{desc['sample_observations']} observations, not the full workload",
                        "pcg_max_iter": cfg["pcg_max_iter"], "pcg_rel_tol": cfg["pcg_rel_tol"], "lambda0": LAMBDA0},
             "cpu_baseline": desc, "gpu_launches": 0, "wall_s": wall,
             "e2e": {"value": value, "unit": "LM iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -254,22 +281,38 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident: warm-up, reset, K timed steps --------------------------------------------
+    # ---- device-resident: warm-up, reset, K timed steps in the library's DEFAULT mode (profiling off: the PCG loop
+    # goes out as CUDA-graph chunks) -> `value`
+    create_stats = gpu.stats()
     run_steps(args.warmup)
     reset()
-    gpu.set_profiling(True)                           # CUDA events around every linearize / matvec launch
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    launches_before = int(gpu.stats().kernels_launched)
     with ClockSampler(local) as clocks:
         start.record()
         steps = run_steps(args.steps)
         stop.record()
         barrier()
     ms = start.elapsed_time(stop)
-    st = gpu.stats()
-    gpu.set_profiling(False)
+    launches_default = int(gpu.stats().kernels_launched) - launches_before
     ms_max = max_over_ranks(ms, dev)
     matvecs = sum(s.pcg_iterations for s in steps)
+
+    # ---- the same K steps again with CUDA events around every linearize / Schur-matvec launch (this switches the
+    # graph chunks off): only the per-kernel averages of the roofline fields come from this pass
+    reset()
+    gpu.set_profiling(True)
+    barrier()
+    start2, stop2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    start2.record()
+    steps_prof = run_steps(args.steps)
+    stop2.record()
+    barrier()
+    ms_prof = start2.elapsed_time(stop2)
+    st = gpu.stats()
+    gpu.set_profiling(False)
+    matvecs_prof = sum(s.pcg_iterations for s in steps_prof)
     lin_count = int(st.linearize_count)
 
     # ---- end to end: host buffers, H2D + lm_step + D2H every step ------------------------------------
@@ -301,7 +344,7 @@ def run_ours(args):
     lin_bytes = 116.0 * n_obs + 48.0 * observed_points
     # launches enqueued after the device-side convergence flag was set return at once (a few us each):
     # their time is kept in the total, but the average is over the matvecs that ran
-    mv_ms = st.matvec_ms_total / max(1, matvecs)
+    mv_ms = st.matvec_ms_total / max(1, matvecs_prof)
     lin_ms = st.linearize_ms_total / max(1, st.linearize_count)
     mv_gbs = mv_bytes / (mv_ms * 1e-3) / 1e9 if mv_ms > 0 else 0.0
     lin_gbs = lin_bytes / (lin_ms * 1e-3) / 1e9 if lin_ms > 0 else 0.0
@@ -322,23 +365,30 @@ def run_ours(args):
         "pcg_iterations": [s.pcg_iterations for s in steps],
         "roofline": {"kernel": "schur_matvec_pipelined_kernel<T>" if st.matvec_pipelined else "schur_pass_kernel<T,MATVEC>", "bound": "hbm", "achieved": mv_gbs, "peak": peak,
                      "unit": "GB/s", "frac": mv_gbs / peak, "traffic": ncu_traffic("schur_matvec") if args.workload == "large" and not args.shrink else None,
+                     "traffic_source": TRAFFIC_FILE + " (ncu --set full, builder run; not measured in this run)",
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": mv_bytes, "avg_launch_ms": mv_ms,
-                     "launches_timed": int(matvecs), "launches_enqueued": int(st.matvec_count), "frac_of_nominal_8TBs": mv_gbs / 8000.0},
-        "roofline_linearize": {"kernel": "linearize_kernel<T,true>", "bound": "hbm", "achieved": lin_gbs, "peak": peak,
+                     "launches_timed": int(matvecs_prof), "launches_enqueued": int(st.matvec_count), "frac_of_nominal_8TBs": mv_gbs / 8000.0,
+                     "timed_in": "second pass of the same K steps with per-launch CUDA events (graph chunks off)"},
+        "roofline_linearize": {"kernel": "linearize_pipelined_kernel<T,NG>" if st.linearize_pipelined else "linearize_kernel<T,true>", "bound": "hbm", "achieved": lin_gbs, "peak": peak,
                                "unit": "GB/s", "frac": lin_gbs / peak, "traffic": ncu_traffic("linearize") if args.workload == "large" and not args.shrink else None,
                                "algorithmic_bytes_per_launch": lin_bytes, "avg_launch_ms": lin_ms,
-                               "launches_timed": lin_count},
+                               "launches_timed": lin_count, "frac_of_nominal_8TBs": lin_gbs / 8000.0},
         "e2e": {"value": world * args.steps / e2e_s, "unit": "LM iterations/s", "h2d_bytes_per_step": param_bytes,
                 "d2h_bytes_per_step": param_bytes + 88,
                 "what": "pinned host parameters -> caspar_ba_set_parameters_host, caspar_ba_lm_step, "
                         "caspar_ba_get_parameters_host + step_info, every step; wall clock"},
-        "gpu_launches": int(st.kernels_launched),
+        "gpu_launches": launches_default,
+        "value_mode": "library default (profiling off, PCG iterations launched as CUDA-graph chunks of 8)",
+        "profiled_pass": {"ms_per_step": ms_prof / args.steps, "lm_iterations_per_s": args.steps / (ms_prof * 1e-3),
+                          "gpu_launches": int(st.kernels_launched)},
+        "create": {"seconds": create_stats.create_seconds, "reorder_seconds": create_stats.reorder_seconds,
+                   "arena_bytes": int(create_stats.arena_bytes),
+                   "what": "caspar_ba_create on this scene (host reordering S0 + uploads), once, untimed"},
         "clocks": clocks.summary(),
     }
     if world == 1 and not args.no_cpu_baseline:
-        v, desc = time_oracle(args.workload, 5, 0, n_obs)          # about 10 s of oracle work on the large sample
-        desc["value"] = v
-        desc["unit"] = "LM iterations/s"
+        desc = time_oracle(args.workload, 5, 0)                    # about 10 s of oracle work on the large sample
+        desc["single_thread"] = time_oracle_single_thread(args.workload)
         line["cpu_baseline"] = desc
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -149,6 +149,7 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.V1 = c.take<float2>(NP);
   v.gp = c.take<float4>(NP);
   v.Vinv = c.take<float4>(2 * NP);
+  v.Vinv64 = c.take<double>(6 * NP);
   v.dp = c.take<float4>(NP);
   v.xp = c.take<double>(3 * NP);
   v.rp = c.take<double>(3 * NP);
@@ -459,6 +460,7 @@ static int create_impl(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba
   v.num_hot = (int)ro.hot_list.size();
   v.robust = pb->robust_loss;
   v.robust_c2 = pb->robust_scale * pb->robust_scale;
+  v.robust_inv_c2 = pb->robust_loss ? 1.0 / ((double)pb->robust_scale * (double)pb->robust_scale) : 0.0;
   v.damping_mode = pb->damping_mode;
   v.camera_model = pb->camera_model;
   v.depth_eps = pb->depth_epsilon;

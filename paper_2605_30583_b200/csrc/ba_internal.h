@@ -69,6 +69,7 @@ struct View {
   int num_chunks;
   int robust;
   float robust_c2;
+  double robust_inv_c2;  // 1 / c^2
   int damping_mode;
   int camera_model;  // 0: angle-axis, additive; 1: Pose3 tangent-space rotation (right perturbation) + retraction
   float depth_eps;   // d_safe = d + eps sign_no_zero(d); 0 = no guard
@@ -109,6 +110,7 @@ struct View {
   float2* V1;             // V_k: yz zz
   float4* gp;             // g_p,k (xyz, w unused)
   float4* Vinv;           // V'^-1, two float4 per point: (xx xy xz yy) (yz zz 0 0) — 32 B, bulk-copy aligned
+  double* Vinv64;         // V'^-1 in fp64, six entries per point (xx xy xz yy yz zz): 48 B, bulk-copy aligned
   float4* dp;             // delta_p,k
   // full-system PCG (N1): point part of the state
   double* xp;             // [3 np] x_p

@@ -170,7 +170,9 @@ __global__ void camera_prepass_kernel(int nc, const float* __restrict__ cams, fl
 // needs is rounded to fp32 once.
 // ------------------------------------------------------------------------------------------------
 struct Projection {
-  float px, py, n, rad, inz, r0, r1;  // p, |p|^2, radial factor, -1/P_z, residual
+  float px, py, n, rad, inz;  // p, |p|^2, radial factor, -1/d_safe
+  double r0, r1;              // residual, fp64: a trial point can throw a two-view point far enough for |r|^2 to
+                              // overflow fp32, while the Cauchy cost of that observation is a few hundred
   float R[9];                         // rotation rounded to fp32 (J_p = A R)
 };
 
@@ -191,8 +193,8 @@ __device__ __forceinline__ Projection project(const float4* __restrict__ row, fl
   const double rad = fma(n, fma((double)k2, n, (double)k1), 1.0);
   const double fr = (double)f * rad;
   Projection o;
-  o.r0 = (float)fma(fr, px, -(double)m.x);
-  o.r1 = (float)fma(fr, py, -(double)m.y);
+  o.r0 = fma(fr, px, -(double)m.x);
+  o.r1 = fma(fr, py, -(double)m.y);
   o.px = (float)px; o.py = (float)py; o.n = (float)n; o.rad = (float)rad; o.inz = (float)inz;
   o.R[0] = (float)a0.x; o.R[1] = (float)a0.y; o.R[2] = (float)a1.x;
   o.R[3] = (float)a1.y; o.R[4] = (float)a2.x; o.R[5] = (float)a2.y;
@@ -205,7 +207,7 @@ __device__ __forceinline__ Projection project(const float4* __restrict__ row, fl
 // respect to the right perturbation R Exp(d) at d = 0, d(R Exp(d) X)/dd = -R [X]x, so J_w = -J_p [X]x = X x J_p(row).
 __device__ __forceinline__ void linearize_observation(const float* __restrict__ table, int cam, float X0, float X1,
                                                       float X2, float2 m, int camera_model, float depth_eps,
-                                                      float (&J)[24], float& r0, float& r1) {
+                                                      float (&J)[24], double& r0, double& r1) {
   const float4* row = reinterpret_cast<const float4*>(table) + 9ll * cam;
   const float4 t6 = __ldg(row + 6), t7 = __ldg(row + 7), t8 = __ldg(row + 8);
   const float f = t6.x, k1 = t6.y, k2 = t6.z, th2 = t6.w;
@@ -269,12 +271,42 @@ __device__ __forceinline__ void linearize_observation(const float* __restrict__ 
 }
 
 __device__ __forceinline__ void residual_observation(const float* __restrict__ table, int cam, float X0, float X1,
-                                                     float X2, float2 m, float depth_eps, float& r0, float& r1) {
+                                                     float X2, float2 m, float depth_eps, double& r0, double& r1) {
   const float4* row = reinterpret_cast<const float4*>(table) + 9ll * cam;
   const float4 t6 = __ldg(row + 6);
   const Projection pr = project(row, t6.x, t6.y, t6.z, X0, X1, X2, m, depth_eps);
   r0 = pr.r0;
   r1 = pr.r1;
+}
+
+// rho(s) of one observation and, with the Cauchy loss, sqrt(w) = (1 + s/c^2)^-1/2 ("robust loss";
+// SURVEY.md O3).  s arrives in fp64; the fp32 fast path covers s/c^2 < 1e30, beyond it (a point thrown to infinity
+// by a trial step) everything is evaluated in fp64 and the Jacobian of that observation, whose weight is < 1e-30,
+// is dropped.
+struct LossTerm {
+  double rho;
+  float sw;    // sqrt(w), 1 without a robust loss
+  bool wild;   // s/c^2 >= 1e30
+};
+
+__device__ __forceinline__ LossTerm loss_term(const View& v, double s2) {
+  LossTerm t;
+  t.rho = s2;
+  t.sw = 1.0f;
+  t.wild = false;
+  if (v.robust) {
+    const double q = s2 * v.robust_inv_c2;
+    if (q < 1e30) {
+      const float qf = (float)q;
+      t.rho = (double)(v.robust_c2 * log1pf(qf));
+      t.sw = sqrtf(1.0f / (1.0f + qf));
+    } else {
+      t.rho = (double)v.robust_c2 * log1p(q);
+      t.sw = (float)rsqrt(1.0 + q);
+      t.wild = true;
+    }
+  }
+  return t;
 }
 
 constexpr int blocks_per_sm(int T) { return T == 128 ? 6 : (T == 192 ? 4 : (T == 256 ? 3 : (T == 512 ? 2 : 1))); }
@@ -355,23 +387,27 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
     __syncthreads();  // the only block-wide barrier: at the start, before anything has latency to expose
   }
 
-  float term = 0.f;
+  double term = 0.0;
   if (JAC) {
     float J[24], r0 = 0.f, r1 = 0.f;
 #pragma unroll
     for (int i = 0; i < 24; ++i) J[i] = 0.f;
     if (cam >= 0) {
-      linearize_observation(table, cam, X.x, X.y, X.z, m, v.camera_model, v.depth_eps, J, r0, r1);
-      const float s2 = fmaf(r0, r0, r1 * r1);
+      double rd0, rd1;
+      linearize_observation(table, cam, X.x, X.y, X.z, m, v.camera_model, v.depth_eps, J, rd0, rd1);
+      const LossTerm lt = loss_term(v, fma(rd0, rd0, rd1 * rd1));
+      term = lt.rho;
+      r0 = (float)rd0; r1 = (float)rd1;
       if (v.robust) {  // Cauchy: w = 1 / (1 + s/c^2), r~ = sqrt(w) r, J~ = sqrt(w) J
-        const float q = s2 / v.robust_c2;
-        const float sw = sqrtf(1.0f / (1.0f + q));
-        term = v.robust_c2 * log1pf(q);
-        r0 *= sw; r1 *= sw;
+        if (!lt.wild) {
+          r0 *= lt.sw; r1 *= lt.sw;
 #pragma unroll
-        for (int i = 0; i < 24; ++i) J[i] *= sw;
-      } else {
-        term = s2;
+          for (int i = 0; i < 24; ++i) J[i] *= lt.sw;
+        } else {
+          r0 = (float)(rd0 * (double)lt.sw); r1 = (float)(rd1 * (double)lt.sw);
+#pragma unroll
+          for (int i = 0; i < 24; ++i) J[i] = 0.f;
+        }
       }
     }
     // eager stores: six 128-bit chunk arrays + the residual, streamed past L2's keep set
@@ -408,17 +444,16 @@ linearize_kernel(View v, const float4* __restrict__ pts, const float* __restrict
     }
   } else {
     if (cam >= 0) {
-      float r0, r1;
+      double r0, r1;
       residual_observation(table, cam, X.x, X.y, X.z, m, v.depth_eps, r0, r1);
-      const float s2 = fmaf(r0, r0, r1 * r1);
-      term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
+      term = loss_term(v, fma(r0, r0, r1 * r1)).rho;
     }
   }
   if (prefetcher) {  // the next wave's points and rank ranges (their tile bounds have long arrived)
     next_thread = prefetch_lines(pts + np0, 16ll * (np1 - np0), next_thread % 64, tid);
     if (JAC) prefetch_lines(v.pt_ptr + np0, 4ll * (np1 - np0 + 1), next_thread % 64, tid);
   }
-  const double wsum = warp_sum((double)term);
+  const double wsum = warp_sum(term);
   if (lane == 0) v.cost_warp[(long long)t * (T / 32) + (tid >> 5)] = wsum;  // folded by reduce_cost_kernel
 }
 
@@ -560,23 +595,27 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(empty + s);
     const long long slot = (long long)t * T + gt;
-    float term = 0.f;
+    double term = 0.0;
     if (JAC) {
       float J[24], r0 = 0.f, r1 = 0.f;
 #pragma unroll
       for (int i = 0; i < 24; ++i) J[i] = 0.f;
       if (cam >= 0) {
-        linearize_observation(table, cam, X.x, X.y, X.z, m, v.camera_model, v.depth_eps, J, r0, r1);
-        const float s2 = fmaf(r0, r0, r1 * r1);
+        double rd0, rd1;
+        linearize_observation(table, cam, X.x, X.y, X.z, m, v.camera_model, v.depth_eps, J, rd0, rd1);
+        const LossTerm lt = loss_term(v, fma(rd0, rd0, rd1 * rd1));
+        term = lt.rho;
+        r0 = (float)rd0; r1 = (float)rd1;
         if (v.robust) {  // Cauchy: w = 1 / (1 + s/c^2), r~ = sqrt(w) r, J~ = sqrt(w) J
-          const float q = s2 / v.robust_c2;
-          const float sw = sqrtf(1.0f / (1.0f + q));
-          term = v.robust_c2 * log1pf(q);
-          r0 *= sw; r1 *= sw;
+          if (!lt.wild) {
+            r0 *= lt.sw; r1 *= lt.sw;
 #pragma unroll
-          for (int i = 0; i < 24; ++i) J[i] *= sw;
-        } else {
-          term = s2;
+            for (int i = 0; i < 24; ++i) J[i] *= lt.sw;
+          } else {
+            r0 = (float)(rd0 * (double)lt.sw); r1 = (float)(rd1 * (double)lt.sw);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) J[i] = 0.f;
+          }
         }
       }
       // eager stores: six 128-bit chunk arrays + the residual, streamed past L2's keep set
@@ -616,13 +655,12 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
       if ((tid & 31) == 0) mbar_arrive(buf_done);  // this warp is done with the buffer
     } else {
       if (cam >= 0) {
-        float r0, r1;
+        double r0, r1;
         residual_observation(table, cam, X.x, X.y, X.z, m, v.depth_eps, r0, r1);
-        const float s2 = fmaf(r0, r0, r1 * r1);
-        term = v.robust ? v.robust_c2 * log1pf(s2 / v.robust_c2) : s2;
+        term = loss_term(v, fma(r0, r0, r1 * r1)).rho;
       }
     }
-    cost_acc += (double)term;
+    cost_acc += term;
     s += NG;
     while (s >= L.stages) { s -= L.stages; ++round; }
   }
@@ -743,18 +781,16 @@ __global__ void __launch_bounds__(128) assemble_schur_diagonal_kernel(View v) {
     const int tile = s / v.T;
     const unsigned pid = v.T <= 256 ? (unsigned)(v.rankpid[s] >> 8) : (v.rankpid32[s] >> 16);
     const long long k = (long long)v.tile_pt[tile] + pid;
-    const float4 vi = __ldg(v.Vinv + 2 * k);
-    const float4 vj = __ldg(v.Vinv + 2 * k + 1);
-    // y = V'^-1 J_p^T (3x2), B = J_p y
-    const float* a = J + 18;  // J_p row 0
-    const float* c = J + 21;  // J_p row 1
-    const float ya0 = fmaf(vi.x, a[0], fmaf(vi.y, a[1], vi.z * a[2])), ya1 = fmaf(vi.y, a[0], fmaf(vi.w, a[1], vj.x * a[2])),
-                ya2 = fmaf(vi.z, a[0], fmaf(vj.x, a[1], vj.y * a[2]));
-    const float yc0 = fmaf(vi.x, c[0], fmaf(vi.y, c[1], vi.z * c[2])), yc1 = fmaf(vi.y, c[0], fmaf(vi.w, c[1], vj.x * c[2])),
-                yc2 = fmaf(vi.z, c[0], fmaf(vj.x, c[1], vj.y * c[2]));
-    const float m00 = 1.0f - fmaf(a[0], ya0, fmaf(a[1], ya1, a[2] * ya2));
-    const float m01 = -fmaf(a[0], yc0, fmaf(a[1], yc1, a[2] * yc2));
-    const float m11 = 1.0f - fmaf(c[0], yc0, fmaf(c[1], yc1, c[2] * yc2));
+    // y = V'^-1 J_p^T (3x2), B = J_p y, in fp64: 1 - B cancels to ~lambda (see schur_pass_kernel)
+    const double* vi = v.Vinv64 + 6 * k;  // xx xy xz yy yz zz
+    const double a[3] = {J[18], J[19], J[20]}, c[3] = {J[21], J[22], J[23]};  // J_p rows
+    const double ya0 = vi[0] * a[0] + vi[1] * a[1] + vi[2] * a[2], ya1 = vi[1] * a[0] + vi[3] * a[1] + vi[4] * a[2],
+                 ya2 = vi[2] * a[0] + vi[4] * a[1] + vi[5] * a[2];
+    const double yc0 = vi[0] * c[0] + vi[1] * c[1] + vi[2] * c[2], yc1 = vi[1] * c[0] + vi[3] * c[1] + vi[4] * c[2],
+                 yc2 = vi[2] * c[0] + vi[4] * c[1] + vi[5] * c[2];
+    const float m00 = (float)(1.0 - (a[0] * ya0 + a[1] * ya1 + a[2] * ya2));
+    const float m01 = (float)(-(a[0] * yc0 + a[1] * yc1 + a[2] * yc2));
+    const float m11 = (float)(1.0 - (c[0] * yc0 + c[1] * yc1 + c[2] * yc2));
     float z0[9], z1[9];  // (I - B) J_c
 #pragma unroll
     for (int q = 0; q < 9; ++q) {
@@ -894,6 +930,7 @@ __global__ void prepare_points_kernel(View v, double lambda) {
     v.step->bad_block = 1;
     v.Vinv[2ll * k] = make_float4(0.f, 0.f, 0.f, 0.f);
     v.Vinv[2ll * k + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = 0; i < 6; ++i) v.Vinv64[6ll * k + i] = 0.0;
     return;
   }
   const double c00 = yy * zz - yz * yz, c01 = xz * yz - xy * zz, c02 = xy * yz - xz * yy;
@@ -901,6 +938,8 @@ __global__ void prepare_points_kernel(View v, double lambda) {
   const double idet = 1.0 / (xx * c00 + xy * c01 + xz * c02);
   v.Vinv[2ll * k] = make_float4((float)(c00 * idet), (float)(c01 * idet), (float)(c02 * idet), (float)(c11 * idet));
   v.Vinv[2ll * k + 1] = make_float4((float)(c12 * idet), (float)(c22 * idet), 0.f, 0.f);
+  double* w = v.Vinv64 + 6ll * k;  // the same inverse unrounded, for the fp64 point elimination
+  w[0] = c00 * idet; w[1] = c01 * idet; w[2] = c02 * idet; w[3] = c11 * idet; w[4] = c12 * idet; w[5] = c22 * idet;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -914,7 +953,15 @@ enum { MATVEC = 0, RHS = 1, BACKSUB = 2 };
 
 template <int T, int MODE>
 __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v) {
-  __shared__ float stage[9][T + 1];
+  // one buffer, two views: pstage[3][T + 1] doubles for the point side, then stage[9][T + 1] floats for the camera side
+  __shared__ double raw[(9 * (T + 1) + 1) / 2];
+  float(*stage)[T + 1] = reinterpret_cast<float(*)[T + 1]>(raw);
+  double(*pstage)[T + 1] = reinterpret_cast<double(*)[T + 1]>(raw);
+  // The point elimination e = u - J_p V'^-1 J_p^T u is a least-squares residual computed through the normal
+  // equations: its rounding error is cond(V'_k) eps |u|, and two-view points with a short baseline have
+  // cond(V') ~ 1e4..1e6.  In fp32 that is 1e-3..1e-1 of |u|, more than the lambda-sized margin that keeps S positive
+  // definite at lambda <= 1e-4: PCG then meets p.Sp <= 0 (skewed).  u, t_k, s_k and e are therefore
+  // carried in fp64 (the stored Jacobians stay fp32; ~35 DFMA per observation, far below the HBM bound).
   __shared__ double red[32];
   const int t = blockIdx.x, tid = threadIdx.x;
   if (MODE == MATVEC) {
@@ -937,7 +984,7 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
     const float4 x = __ldcs(&v.J[c][slot]);  // streamed once per pass: evict-first
     J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
   }
-  float u0 = 0.f, u1 = 0.f;
+  double u0 = 0.0, u1 = 0.0;
   if (MODE != RHS) {
     if (cam >= 0) {
       const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
@@ -945,39 +992,37 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
       const float pj[9] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x};
 #pragma unroll
       for (int i = 0; i < 9; ++i) {
-        u0 = fmaf(J[i], pj[i], u0);
-        u1 = fmaf(J[9 + i], pj[i], u1);
+        u0 = fma((double)J[i], (double)pj[i], u0);
+        u1 = fma((double)J[9 + i], (double)pj[i], u1);
       }
-      stage[0][rank] = fmaf(J[18], u0, J[21] * u1);
-      stage[1][rank] = fmaf(J[19], u0, J[22] * u1);
-      stage[2][rank] = fmaf(J[20], u0, J[23] * u1);
+      pstage[0][rank] = fma((double)J[18], u0, (double)J[21] * u1);
+      pstage[1][rank] = fma((double)J[19], u0, (double)J[22] * u1);
+      pstage[2][rank] = fma((double)J[20], u0, (double)J[23] * u1);
     }
     __syncthreads();
   }
   // point threads
-  float dg_part = 0.f;
+  double dg_part = 0.0;
   for (int k = p0 + tid; k < p1; k += T) {
     const int rb = v.pt_ptr[k] - base, re = v.pt_ptr[k + 1] - base;
-    float t0 = 0.f, t1 = 0.f, t2 = 0.f;
+    double t0 = 0.0, t1 = 0.0, t2 = 0.0;
     if (MODE != RHS)
-      for (int r = rb; r < re; ++r) { t0 += stage[0][r]; t1 += stage[1][r]; t2 += stage[2][r]; }
-    const float4 vi = v.Vinv[2ll * k];
-    const float4 vj = v.Vinv[2ll * k + 1];
+      for (int r = rb; r < re; ++r) { t0 += pstage[0][r]; t1 += pstage[1][r]; t2 += pstage[2][r]; }
+    const double* vi = v.Vinv64 + 6ll * k;  // xx xy xz yy yz zz
     float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
     if (MODE != MATVEC) {
       g = v.gp[k];
       t0 += g.x; t1 += g.y; t2 += g.z;
     }
-    float s0 = fmaf(vi.x, t0, fmaf(vi.y, t1, vi.z * t2));
-    float s1 = fmaf(vi.y, t0, fmaf(vi.w, t1, vj.x * t2));
-    float s2 = fmaf(vi.z, t0, fmaf(vj.x, t1, vj.y * t2));
+    double s0 = vi[0] * t0 + vi[1] * t1 + vi[2] * t2;
+    double s1 = vi[1] * t0 + vi[3] * t1 + vi[4] * t2;
+    double s2 = vi[2] * t0 + vi[4] * t1 + vi[5] * t2;
     if (MODE == BACKSUB) {
       s0 = -s0; s1 = -s1; s2 = -s2;
-      v.dp[k] = make_float4(s0, s1, s2, 0.f);
-      dg_part += fmaf(s0, g.x, fmaf(s1, g.y, s2 * g.z));
+      v.dp[k] = make_float4((float)s0, (float)s1, (float)s2, 0.f);
+      dg_part += s0 * g.x + s1 * g.y + s2 * g.z;
     }
-
-    for (int r = rb; r < re; ++r) { stage[0][r] = s0; stage[1][r] = s1; stage[2][r] = s2; }
+    for (int r = rb; r < re; ++r) { pstage[0][r] = s0; pstage[1][r] = s1; pstage[2][r] = s2; }
   }
   __syncthreads();
   float c9[9];
@@ -985,22 +1030,23 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
 #pragma unroll
   for (int i = 0; i < 9; ++i) c9[i] = 0.f;
   if (cam >= 0) {
-    const float s0 = stage[0][rank], s1 = stage[1][rank], s2 = stage[2][rank];
-    const float w0 = fmaf(J[18], s0, fmaf(J[19], s1, J[20] * s2));
-    const float w1 = fmaf(J[21], s0, fmaf(J[22], s1, J[23] * s2));
+    const double s0 = pstage[0][rank], s1 = pstage[1][rank], s2 = pstage[2][rank];
+    const double w0 = (double)J[18] * s0 + (double)J[19] * s1 + (double)J[20] * s2;
+    const double w1 = (double)J[21] * s0 + (double)J[22] * s1 + (double)J[23] * s2;
     if (MODE == BACKSUB) {
-      const float y0 = u0 + w0, y1 = u1 + w1;  // (J delta)_i
-      dot_part = (double)y0 * (double)y0 + (double)y1 * (double)y1;
+      const double y0 = u0 + w0, y1 = u1 + w1;  // (J delta)_i
+      dot_part = y0 * y0 + y1 * y1;
     } else {
-      const float e0 = (MODE == MATVEC) ? u0 - w0 : w0;
-      const float e1 = (MODE == MATVEC) ? u1 - w1 : w1;
-      if (MODE == MATVEC) dot_part = (double)u0 * (double)e0 + (double)u1 * (double)e1;
+      const double ed0 = (MODE == MATVEC) ? u0 - w0 : w0;
+      const double ed1 = (MODE == MATVEC) ? u1 - w1 : w1;
+      if (MODE == MATVEC) dot_part = u0 * ed0 + u1 * ed1;
+      const float e0 = (float)ed0, e1 = (float)ed1;
 #pragma unroll
       for (int i = 0; i < 9; ++i) c9[i] = fmaf(J[i], e0, J[9 + i] * e1);
     }
   }
   if (MODE != BACKSUB) {
-    __syncthreads();  // every thread has read its s_k
+    __syncthreads();  // every thread has read its s_k: the buffer becomes the camera-side staging rows
 #pragma unroll
     for (int i = 0; i < 9; ++i) stage[i][tid] = c9[i];
     __syncthreads();
@@ -1021,7 +1067,7 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
   }
   if (MODE == BACKSUB) {
     const double jd2 = block_sum(dot_part, red);
-    const double dg = block_sum((double)dg_part, red);
+    const double dg = block_sum(dg_part, red);
     if (tid == 0) {
       atomicAdd(&v.step->jd2, jd2);
       atomicAdd(&v.step->dg, dg);
@@ -1062,10 +1108,10 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   L.cam = L.j + 6 * T * 16;
   L.rank = L.cam + T * 4;
   L.vinv = up(L.rank + T * 2);
-  L.meta = up(L.vinv + max_pts * 32);
+  L.meta = up(L.vinv + max_pts * 48);  // V'^-1 in fp64, six entries per point
   L.stage_bytes = up(L.meta + meta_max);
-  L.tbuf_bytes = up(3 * (T + 2) * 4);
-  L.sbuf_bytes = up(3 * (T + 1) * 4);
+  L.tbuf_bytes = up(3 * (T + 2) * 8);  // the point side is carried in fp64 (see schur_pass_kernel)
+  L.sbuf_bytes = up(3 * (T + 1) * 8);
   const int hot_bytes = up(num_hot * 9 * 8);  // per-CTA fp64 accumulators of the hot cameras' q rows
   const int fixed = NG * (L.tbuf_bytes + L.sbuf_bytes) + NG * (T / 32) * kWarpScratchBytes + hot_bytes + 256;
   int st = (smem_limit - fixed) / L.stage_bytes;
@@ -1129,14 +1175,14 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         const int4 dn = tn < v.num_tiles ? __ldg(v.tile_dir + tn) : make_int4(0, 0, 0, 0);  // prefetch next entry
         mbar_wait(empty + s, ph ^ 1);
         unsigned char* st = smem + (size_t)s * L.stage_bytes;
-        const unsigned vinv_bytes = (unsigned)d.w * 32u;
+        const unsigned vinv_bytes = (unsigned)d.w * 48u;
         mbar_expect_tx(full + s, (unsigned)(6 * T * 16 + T * 4 + T * 2) + vinv_bytes + (unsigned)d.y);
         const long long slot0 = (long long)t * T;
 #pragma unroll
         for (int c = 0; c < 6; ++c) bulk_g2s(st + L.j + c * T * 16, v.J[c] + slot0, T * 16, full + s, pol_stream);
         bulk_g2s(st + L.cam, v.cam + slot0, T * 4, full + s, pol_stream);
         bulk_g2s(st + L.rank, v.rankpid + slot0, T * 2, full + s, pol_stream);
-        bulk_g2s(st + L.vinv, v.Vinv + 2ll * d.z, vinv_bytes, full + s, pol_keep);
+        bulk_g2s(st + L.vinv, v.Vinv64 + 6ll * d.z, vinv_bytes, full + s, pol_keep);
         bulk_g2s(st + L.meta, v.tile_meta + 16ll * d.x, (unsigned)d.y, full + s, pol_stream);
         d = dn;
         if (++s == L.stages) { s = 0; ph ^= 1; }
@@ -1149,8 +1195,8 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   const int g = tid / T, gt = tid - g * T, lane = tid & 31;
   const int bar_id = 1 + g;
   // row stride T + 2: the six lanes of a point in phase B (component c, half h) read banks 2c + h + rank: distinct
-  float(*tbuf)[T + 2] = reinterpret_cast<float(*)[T + 2]>(smem + L.tbuf + (size_t)g * L.tbuf_bytes);  // by rank
-  float(*sbuf)[T + 1] = reinterpret_cast<float(*)[T + 1]>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // by point
+  double(*tbuf)[T + 2] = reinterpret_cast<double(*)[T + 2]>(smem + L.tbuf + (size_t)g * L.tbuf_bytes);  // by rank
+  double(*sbuf)[T + 1] = reinterpret_cast<double(*)[T + 1]>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // by point
   float* rows = reinterpret_cast<float*>(smem + L.scratch + (size_t)(tid >> 5) * kWarpScratchBytes);
   int* camrow = reinterpret_cast<int*>(rows + 9 * 33);
   // p.q = sum_i u_i.e_i (+ p.lambda D_c p, added by the update kernel): the curvature of the operator AS COMPUTED,
@@ -1176,7 +1222,12 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
       pa = __ldg(pv); pb = __ldg(pv + 1); pc = __ldg(pv + 2);
     }
-    float u0 = 0.f, u1 = 0.f;
+    // The point elimination (t_k, s_k, e) is carried in fp64: its rounding error is cond(V'_k) eps |u|, and in
+    // fp32 that exceeds the lambda-sized margin that keeps S positive definite once lambda <= 1e-4 (see
+    // schur_pass_kernel).  u itself stays an fp32 dot product: an error du in u passes through the
+    // projection I - B as (I - B) du, it is not amplified (and every fp32 -> fp64 conversion is a quarter-rate
+    // XU instruction: converting the 18 entries of J_c per observation cost 0.14 ms per matvec).
+    float uf0 = 0.f, uf1 = 0.f;
     float Jp[6];
     {
       float J[24];
@@ -1188,16 +1239,20 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       const float pj[9] = {pa.x, pa.y, pa.z, pa.w, pb.x, pb.y, pb.z, pb.w, pc.x};
 #pragma unroll
       for (int k = 0; k < 9; ++k) {
-        u0 = fmaf(J[k], pj[k], u0);
-        u1 = fmaf(J[9 + k], pj[k], u1);
+        uf0 = fmaf(J[k], pj[k], uf0);
+        uf1 = fmaf(J[9 + k], pj[k], uf1);
       }
 #pragma unroll
       for (int k = 0; k < 6; ++k) Jp[k] = J[18 + k];
     }
+    const double u0 = (double)uf0, u1 = (double)uf1;
+    double Jpd[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) Jpd[k] = (double)Jp[k];
     if (cam >= 0) {
-      tbuf[0][rank] = fmaf(Jp[0], u0, Jp[3] * u1);
-      tbuf[1][rank] = fmaf(Jp[1], u0, Jp[4] * u1);
-      tbuf[2][rank] = fmaf(Jp[2], u0, Jp[5] * u1);
+      tbuf[0][rank] = fma(Jpd[0], u0, Jpd[3] * u1);
+      tbuf[1][rank] = fma(Jpd[1], u0, Jpd[4] * u1);
+      tbuf[2][rank] = fma(Jpd[2], u0, Jpd[5] * u1);
     }
     group_bar(bar_id, T);
     // ---- phase B: six lanes per point (component x half of the track; lanes 30, 31 idle, five points per
@@ -1208,25 +1263,23 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         const int k = k0 + lp;
         const bool valid = lane < 30 && k < npts;
         const int rb = valid ? pt_start[k] : 0, re = valid ? pt_start[k + 1] : 0;
-        float tsum = 0.f;
+        double tsum = 0.0;
         for (int r = rb + half; r < re; r += 8) {  // four independent loads per round
-          const float a0 = tbuf[c][r];
-          const float a1 = r + 2 < re ? tbuf[c][r + 2] : 0.f;
-          const float a2 = r + 4 < re ? tbuf[c][r + 4] : 0.f;
-          const float a3 = r + 6 < re ? tbuf[c][r + 6] : 0.f;
+          const double a0 = tbuf[c][r];
+          const double a1 = r + 2 < re ? tbuf[c][r + 2] : 0.0;
+          const double a2 = r + 4 < re ? tbuf[c][r + 4] : 0.0;
+          const double a3 = r + 6 < re ? tbuf[c][r + 6] : 0.0;
           tsum += (a0 + a1) + (a2 + a3);
         }
         tsum += __shfl_xor_sync(0xffffffffu, tsum, 1);
         const int base = 6 * lp;
-        const float t0 = __shfl_sync(0xffffffffu, tsum, base), t1 = __shfl_sync(0xffffffffu, tsum, base + 2),
-                    t2 = __shfl_sync(0xffffffffu, tsum, base + 4);
+        const double t0 = __shfl_sync(0xffffffffu, tsum, base), t1 = __shfl_sync(0xffffffffu, tsum, base + 2),
+                     t2 = __shfl_sync(0xffffffffu, tsum, base + 4);
         if (valid && half == 0) {
-          const float4 vi = reinterpret_cast<const float4*>(st + L.vinv)[2 * k];      // xx xy xz yy
-          const float2 vj = reinterpret_cast<const float2*>(st + L.vinv)[4 * k + 2];  // yz zz
-          const float m0 = c == 0 ? vi.x : (c == 1 ? vi.y : vi.z);
-          const float m1 = c == 0 ? vi.y : (c == 1 ? vi.w : vj.x);
-          const float m2 = c == 0 ? vi.z : (c == 1 ? vj.x : vj.y);
-          sbuf[c][k] = fmaf(m0, t0, fmaf(m1, t1, m2 * t2));
+          const double* vi = reinterpret_cast<const double*>(st + L.vinv) + 6 * k;  // xx xy xz yy yz zz
+          // row c of the symmetric 3x3: (0: xx xy xz) (1: xy yy yz) (2: xz yz zz)
+          const double m0 = vi[c], m1 = vi[c == 0 ? 1 : (c == 1 ? 3 : 4)], m2 = vi[c == 0 ? 2 : (c == 1 ? 4 : 5)];
+          sbuf[c][k] = m0 * t0 + m1 * t1 + m2 * t2;
         }
       }
     }
@@ -1236,10 +1289,12 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     {
       float e0 = 0.f, e1 = 0.f;
       if (cam >= 0) {
-        const float s0 = sbuf[0][pid], s1 = sbuf[1][pid], s2 = sbuf[2][pid];
-        e0 = u0 - fmaf(Jp[0], s0, fmaf(Jp[1], s1, Jp[2] * s2));
-        e1 = u1 - fmaf(Jp[3], s0, fmaf(Jp[4], s1, Jp[5] * s2));
-        dot_part += (double)fmaf(u0, e0, u1 * e1);  // O(1) magnitudes (the direction is normalised): no underflow
+        const double s0 = sbuf[0][pid], s1 = sbuf[1][pid], s2 = sbuf[2][pid];
+        const double ed0 = u0 - (Jpd[0] * s0 + Jpd[1] * s1 + Jpd[2] * s2);
+        const double ed1 = u1 - (Jpd[3] * s0 + Jpd[4] * s1 + Jpd[5] * s2);
+        dot_part += u0 * ed0 + u1 * ed1;
+        e0 = (float)ed0;
+        e1 = (float)ed1;
       }
       float J[20];  // J_c again, from the stage (cheaper than 18 registers held across two barriers)
 #pragma unroll

@@ -6,6 +6,12 @@ import pytest
 from ba_scenes import CONFIGS, make_scene, scene_summary
 
 
+@pytest.mark.parametrize("name", ["tiny", "small", "mid"])
+def test_full_observation_table(scene_cache, name):
+    from ba_scenes import FULL_OBSERVATIONS
+    assert scene_cache(name).num_observations == FULL_OBSERVATIONS[name]   # large / skewed: tests/test_gpu_golden.py
+
+
 def test_tiny_counts(scene_cache):
     s = scene_cache("tiny")
     m = scene_summary(s)

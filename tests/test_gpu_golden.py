@@ -6,8 +6,9 @@ tests/golden/fullsize_<config>.npz was written by tests/golden/make_fullsize_gol
 on the seeded scene of `ba_scenes/` (minutes of fp64 CPU work per config; nothing in it comes from the CUDA path).
 Tolerances are north_star's (C12 / C13): blocks 1e-5, gradient / Schur right-hand side / Schur matvec /
 PCG step 1e-4 in L2 -- taken PER PARAMETER CLASS (rotation, translation, f, k1, k2) as well as globally -- and the
-cost after every step of the config's own LM schedule (PCG cap 100, tol 1e-10: C16) to 1e-4 where the oracle's
-linear solve is resolved; where it is not, the bound DESIGN.md C17 states from the measured table."""
+cost after EVERY step of the config's own LM schedule (PCG cap 100, tol 1e-10: C16) to 1e-4, whether or not the
+oracle's linear solve is resolved at that step (measured: <= 3e-7 on mid and large, <= 6e-5 on skewed, whose PCG
+stalls at 0.1-3 |b| from step 10 on: DESIGN.md C17)."""
 import hashlib
 import json
 import os
@@ -23,9 +24,9 @@ pytestmark = pytest.mark.gpu
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 REPORT = os.path.join(os.path.dirname(GOLDEN), "..", "gpurun_out")
 
-# DESIGN.md C17: cost gate of a replayed step by the oracle's own PCG residual at that step
-RESOLVED = 1e-2          # |r|/|b| <= 1e-2: the solve is resolved, the cost is compared at north_star's 1e-4
-UNRESOLVED_COST_TOL = {"mid": 1e-4, "large": 1e-4, "skewed": 2e-2}
+# DESIGN.md C17: the final cameras are compared where every linear solve of the schedule was resolved by the oracle
+RESOLVED = 1e-2          # |r|/|b| <= 1e-2
+COST_TOL = 1e-4          # north_star, every step of every config
 
 
 def _sha(a):
@@ -43,6 +44,8 @@ def full(request, scene_cache):
     s = scene_cache(name)
     # the scene must be the one the oracle saw
     assert list(gold["fp_counts"]) == [s.num_cameras, s.num_points, s.num_observations]
+    from ba_scenes import FULL_OBSERVATIONS
+    assert s.num_observations == FULL_OBSERVATIONS[name]
     assert str(gold["fp_sha_camera_index"]) == _sha(s.camera_index)
     assert str(gold["fp_sha_point_index"]) == _sha(s.point_index)
     sums = np.array([np.abs(s.cameras.astype(np.float64)).sum(), np.abs(s.points.astype(np.float64)).sum(),
@@ -147,13 +150,13 @@ def test_lm_schedule_against_the_golden(full):
                              cost_before_err=eb, cost_after_err=ea, rho_gpu=got.rho, rho_oracle=float(gold["sched_rho"][t])))
             resolved = res_o <= RESOLVED
             resolved_all &= resolved
-            bound = 1e-4 if resolved else UNRESOLVED_COST_TOL[name]
-            assert eb <= bound and ea <= bound, rows[-1]
+            assert eb <= COST_TOL and ea <= COST_TOL, rows[-1]
     finally:
         full["report"]["schedule"] = rows
-    if resolved_all:
-        cams = g.cameras.cpu().numpy().astype(np.float64)
-        errs = per_class_rel_l2(cams, gold["final_cameras"])
-        full["report"]["final_cameras"] = errs
+    cams = g.cameras.cpu().numpy().astype(np.float64)
+    errs = per_class_rel_l2(cams, gold["final_cameras"])
+    full["report"]["final_cameras"] = errs
+    full["report"]["all_solves_resolved"] = bool(resolved_all)
+    if resolved_all:      # otherwise the end point of 20 unconverged solves is not unique to 1e-4 (recorded only)
         assert max(errs.values()) <= 1e-4, errs
     g.close()

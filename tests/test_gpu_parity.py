@@ -146,11 +146,12 @@ def test_pcg_tolerance_stop_matches_oracle(pair):
 
 # ------------------------------------------------------------------ S1-S10 replayed LM schedule
 # DESIGN.md C17: a replayed step is gated at north_star's 1e-4 while the ORACLE's own linear solve is resolved
-# (|r|/|b| <= 1e-2 at the config's cap); past that an unconverged CG iterate is a chaotic function of rounding, and
-# the step is gated at the bound the measured table in DESIGN.md C17 supports (skewed only; every other config
-# stays at 1e-4 for all of its steps).
+# (|r|/|b| <= 1e-2 at the config's cap).  Past that an unconverged CG iterate is a sensitive function of rounding;
+# only the SHRUNKEN skewed scene (300 cameras: every camera sees a tenth of the points, the oracle's PCG stalls at
+# 0.1-0.9 |b| for most of the schedule) needs the allowance, 1e-3 (measured 3.9e-4); the full-size configs,
+# skewed included, hold 1e-4 at every step (tests/test_gpu_golden.py).
 RESOLVED = 1e-2
-UNRESOLVED_COST_TOL = {"tiny": 1e-4, "small": 1e-4, "mid": 1e-4, "large": 1e-4, "skewed": 2e-2}
+UNRESOLVED_COST_TOL = {"tiny": 1e-4, "small": 1e-4, "mid": 1e-4, "large": 1e-4, "skewed": 1e-3}
 
 
 @pytest.mark.parametrize("key", list(SCENES))
