@@ -30,6 +30,32 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIBRARY
 
 
+def ptxas_table() -> str:
+    """Registers / stack / spills / static shared memory of every kernel, from `nvcc -Xptxas -v` (evidence for
+    profiles/: `python -m paper_2605_30583_b200.build --ptxas-table`)."""
+    import re
+    import tempfile
+
+    rows = []
+    with tempfile.TemporaryDirectory() as tmp:
+        cmd = [NVCC, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xptxas", "-v",
+               "-c", "ba_kernels.cu", "-o", os.path.join(tmp, "k.o")]
+        txt = subprocess.run(cmd, check=True, cwd=CSRC, capture_output=True, text=True).stderr
+    pat = re.compile(r"Compiling entry function '([^']+)'.*?\n.*?\n\s+(\d+) bytes stack frame, (\d+) bytes spill stores, "
+                     r"(\d+) bytes spill loads\n.*?Used (\d+) registers(?:, used (\d+) barriers)?(?:, (\d+) bytes smem)?")
+    ents = pat.findall(txt)
+    names = subprocess.run(["c++filt"] + [e[0] for e in ents], capture_output=True, text=True).stdout.splitlines()
+    rows.append("| kernel | registers | stack B | spill stores / loads B | static smem B |")
+    rows.append("|---|---|---|---|---|")
+    for n, e in zip(names, ents):
+        n = re.sub(r"\(.*", "", n.replace("cba::", "").replace("void ", ""))
+        rows.append(f"| `{n}` | {e[4]} | {e[1]} | {e[2]} / {e[3]} | {e[6] or 0} |")
+    return "\n".join(rows)
+
+
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    if "--ptxas-table" in sys.argv:
+        print(ptxas_table())
+    else:
+        print(build(force=True, verbose="-v" in sys.argv))

@@ -86,6 +86,15 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
       : "memory");
 }
 
+// A consumer that has read a stage with ordinary (generic-proxy) shared-memory loads must order those reads before
+// the bulk copy (async proxy) that refills the stage: the release of mbarrier.arrive alone does not reach across
+// proxies.  Without this fence a warp whose gathered loads were still queued when its lane 0 arrived on the `empty`
+// barrier read a few rows of the NEXT tile's points about once in 10^7 warp-tiles (measured on the skewed scene:
+// 22 of 400 linearize calls had one warp of wrong residuals).  Every reading thread executes it.
+__device__ __forceinline__ void fence_reads_before_refill() {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
 __device__ __forceinline__ void group_bar(int id, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
@@ -591,7 +600,9 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
         p0 = reinterpret_cast<const int*>(st + L.meta)[3];
       }
     }
-    // everything this thread needs from the stage is in registers: hand it back to the producer
+    // everything this thread needs from the stage has been read (not necessarily returned: X and the rank range
+    // are first used far below), so the reads are fenced against the refill before the stage is handed back
+    fence_reads_before_refill();
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(empty + s);
     const long long slot = (long long)t * T + gt;
@@ -1305,9 +1316,6 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
 #pragma unroll
       for (int k = 0; k < 9; ++k) c9[k] = fmaf(J[k], e0, J[9 + k] * e1);
     }
-    // this warp is done with the stage
-    __syncwarp();
-    if (lane == 0) mbar_arrive(empty + s);
     // ---- camera side, warp-local.  The tile's slots are sorted by camera, so a warp holds whole pieces of
     // camera runs (lane intervals).  The nine products go to the warp's scratch rows (bank = component + lane:
     // conflict free); lane (k, part) then walks component k over slots [11 part, 11 part + 11) and adds a
@@ -1321,6 +1329,13 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       for (int k = 0; k < 9; ++k) rows[k * 33 + lane] = c9[k];
       camrow[lane] = cam;
       __syncwarp();
+      // This warp is done with the stage.  The release sits HERE, after the scratch-row stores, on purpose: every
+      // value this warp loaded from the stage has by now been consumed by an instruction whose result one of
+      // those stores needs, so no stage read can still be queued when the producer's bulk copy (async proxy)
+      // refills it.  Releasing right after the last stage load raced (see fence_reads_before_refill; the
+      // linearize kernel, which releases early, needs the proxy fence); the fence here instead of the data
+      // dependence measured 0.753 against 0.738 ms per matvec on Large.
+      if (lane == 0) mbar_arrive(empty + s);
       if (lane < 27) {
         const int part = lane / 9, k = lane - 9 * part, s0 = 11 * part;
         const float* src = rows + k * 33 + s0;

@@ -104,6 +104,27 @@ def test_linearize_against_the_golden(full):
     assert rep["V"] <= 1e-5 and errv.max() <= 1e-4   # per block: short fp32 sums of <= 200 terms
 
 
+def test_linearize_repeats_bit_for_bit_at_full_size(full):
+    """Stress repeat of S2+S3 in the bench launch configuration: the cost (an fp64 sum in a fixed order over every
+    observation) must come back with the same BITS on every call.  This is the test that catches a stage of the TMA
+    ring being refilled while a lagging warp still reads it: before the proxy fence in linearize_pipelined_kernel
+    22 of 400 calls on the skewed scene had one warp of wrong residuals, i.e. a miss probability of
+    < 0.5 % at 100 calls."""
+    g, torch = full["gpu"], full["torch"]
+    calls = 100 if full["name"] == "skewed" else 40
+    ref = g.export_device(pkg.RESIDUALS).clone()
+    costs = {g.linearize() for _ in range(calls)}
+    assert costs == {full["cost"]}, sorted(costs)
+    assert torch.equal(g.export_device(pkg.RESIDUALS), ref)
+    q0 = g.schur_matvec(float(full["gold"]["lam1"]), full["gold"]["p1"].astype(np.float64))
+    worst = 0.0
+    for _ in range(calls):            # q = S p: the order of the fp64 REDs is free (C14), a wrong warp is not
+        q = g.schur_matvec(float(full["gold"]["lam1"]), full["gold"]["p1"].astype(np.float64))
+        worst = max(worst, rel_l2(q, q0))
+    full["report"]["matvec_repeat_worst"] = worst
+    assert worst <= 1e-12, worst
+
+
 def test_schur_matvec_against_the_golden(full):
     g, gold = full["gpu"], full["gold"]
     for tag in ("1", "2"):
