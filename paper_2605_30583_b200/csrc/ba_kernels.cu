@@ -1238,8 +1238,11 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     // schur_pass_kernel).  u itself stays an fp32 dot product: an error du in u passes through the
     // projection I - B as (I - B) du, it is not amplified (and every fp32 -> fp64 conversion is a quarter-rate
     // XU instruction: converting the 18 entries of J_c per observation cost 0.14 ms per matvec).
+    // J_c stays in registers across the two group barriers (18 registers); J_p is converted for the point side,
+    // dropped, and re-read from the stage in phase C: two 128-bit loads instead of the five that re-reading J_c
+    // took (the kernel is bound by shared-memory wavefronts: profiles/r02_ncu_schur_matvec.md).
     float uf0 = 0.f, uf1 = 0.f;
-    float Jp[6];
+    float Jc[18];
     {
       float J[24];
 #pragma unroll
@@ -1254,16 +1257,13 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         uf1 = fmaf(J[9 + k], pj[k], uf1);
       }
 #pragma unroll
-      for (int k = 0; k < 6; ++k) Jp[k] = J[18 + k];
-    }
-    const double u0 = (double)uf0, u1 = (double)uf1;
-    double Jpd[6];
-#pragma unroll
-    for (int k = 0; k < 6; ++k) Jpd[k] = (double)Jp[k];
-    if (cam >= 0) {
-      tbuf[0][rank] = fma(Jpd[0], u0, Jpd[3] * u1);
-      tbuf[1][rank] = fma(Jpd[1], u0, Jpd[4] * u1);
-      tbuf[2][rank] = fma(Jpd[2], u0, Jpd[5] * u1);
+      for (int k = 0; k < 18; ++k) Jc[k] = J[k];
+      if (cam >= 0) {
+        const double u0 = (double)uf0, u1 = (double)uf1;
+        tbuf[0][rank] = fma((double)J[18], u0, (double)J[21] * u1);
+        tbuf[1][rank] = fma((double)J[19], u0, (double)J[22] * u1);
+        tbuf[2][rank] = fma((double)J[20], u0, (double)J[23] * u1);
+      }
     }
     group_bar(bar_id, T);
     // ---- phase B: six lanes per point (component x half of the track; lanes 30, 31 idle, five points per
@@ -1300,21 +1300,18 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     {
       float e0 = 0.f, e1 = 0.f;
       if (cam >= 0) {
+        const float4 x4 = reinterpret_cast<const float4*>(st + L.j + 4 * T * 16)[gt];  // Jc16 Jc17 Jp0 Jp1
+        const float4 x5 = reinterpret_cast<const float4*>(st + L.j + 5 * T * 16)[gt];  // Jp2 .. Jp5
+        const double u0 = (double)uf0, u1 = (double)uf1;
         const double s0 = sbuf[0][pid], s1 = sbuf[1][pid], s2 = sbuf[2][pid];
-        const double ed0 = u0 - (Jpd[0] * s0 + Jpd[1] * s1 + Jpd[2] * s2);
-        const double ed1 = u1 - (Jpd[3] * s0 + Jpd[4] * s1 + Jpd[5] * s2);
+        const double ed0 = u0 - ((double)x4.z * s0 + (double)x4.w * s1 + (double)x5.x * s2);
+        const double ed1 = u1 - ((double)x5.y * s0 + (double)x5.z * s1 + (double)x5.w * s2);
         dot_part += u0 * ed0 + u1 * ed1;
         e0 = (float)ed0;
         e1 = (float)ed1;
       }
-      float J[20];  // J_c again, from the stage (cheaper than 18 registers held across two barriers)
 #pragma unroll
-      for (int c = 0; c < 5; ++c) {
-        const float4 x = reinterpret_cast<const float4*>(st + L.j + c * T * 16)[gt];
-        J[4 * c] = x.x; J[4 * c + 1] = x.y; J[4 * c + 2] = x.z; J[4 * c + 3] = x.w;
-      }
-#pragma unroll
-      for (int k = 0; k < 9; ++k) c9[k] = fmaf(J[k], e0, J[9 + k] * e1);
+      for (int k = 0; k < 9; ++k) c9[k] = fmaf(Jc[k], e0, Jc[9 + k] * e1);
     }
     // ---- camera side, warp-local.  The tile's slots are sorted by camera, so a warp holds whole pieces of
     // camera runs (lane intervals).  The nine products go to the warp's scratch rows (bank = component + lane:
