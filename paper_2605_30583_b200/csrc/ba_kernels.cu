@@ -505,7 +505,9 @@ __host__ __device__ inline LinLayout lin_layout(int T, int NG, int max_pts, int 
   L.sbuf_bytes = jac ? 2 * up(T * 40) : 0;  // per group, x2 buffers: float4 stage[T][2], float gz[T], unsigned arrived[T]
   const int fixed = NG * L.sbuf_bytes + 512;  // 512: full[12], empty[12], seen[12], done[2 NG]
   int st = (smem_limit - fixed) / L.stage_bytes;
-  if (st > 8) st = 8;  // 8 tiles of inputs (~50 KB) in flight per SM is far more than the consumers can drain
+  const int cap = NG == 3 ? 9 : 2 * NG;  // 8 - 12 tiles of inputs (<= 55 KB at T = 256) in flight per SM: far more than the consumers drain
+  if (st > cap) st = cap;
+  if (st >= NG) st -= st % NG;  // a multiple of NG: every stage belongs to one group, no `seen` guard (see the matvec)
   L.stages = st;
   L.sbuf = L.stages * L.stage_bytes;
   L.bars = L.sbuf + NG * L.sbuf_bytes;
@@ -574,15 +576,19 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
   int s = g % L.stages;
   int round = g / L.stages;
   int k = 0;  // tiles this group has done
+  const bool guard = (L.stages % NG) != 0;
   for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G, ++k) {
     unsigned char* sb = smem + L.sbuf + (size_t)(2 * g + (k & 1)) * (L.sbuf_bytes / 2);  // this tile's buffer
-    float4(*stage)[2] = reinterpret_cast<float4(*)[2]>(sb);         // by rank: (Vxx Vxy Vxz Vyy) (Vyz Vzz gx gy)
+    // by rank, two arrays of 16-byte rows (one array of 32-byte rows put rows r and r + 4 on the same banks):
+    float4* stage_a = reinterpret_cast<float4*>(sb);                // (Vxx Vxy Vxz Vyy)
+    float4* stage_b = reinterpret_cast<float4*>(sb + T * 16);       // (Vyz Vzz gx gy)
     float* stage_gz = reinterpret_cast<float*>(sb + T * 32);        // by rank: gz
     unsigned* arrived = reinterpret_cast<unsigned*>(sb + T * 36);   // by local point id
-    while (seen[s] < round) {
-    }
+    if (guard)
+      while (seen[s] < round) {
+      }
     mbar_wait(full + s, (unsigned)(round & 1));
-    if (gt == 0) seen[s] = round + 1;
+    if (guard && gt == 0) seen[s] = round + 1;
     const unsigned char* st = smem + (size_t)s * L.stage_bytes;
     const int cam = reinterpret_cast<const int*>(st + L.cam)[gt];
     const unsigned rp = reinterpret_cast<const unsigned short*>(st + L.rank)[gt];
@@ -637,10 +643,10 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
       unsigned long long* buf_done = done + 2 * g + (k & 1);
       if (k >= 2) mbar_wait(buf_done, (unsigned)(((k >> 1) - 1) & 1));
       if (cam >= 0) {
-        stage[rank][0] = make_float4(fmaf(J[18], J[18], J[21] * J[21]), fmaf(J[18], J[19], J[21] * J[22]),
-                                     fmaf(J[18], J[20], J[21] * J[23]), fmaf(J[19], J[19], J[22] * J[22]));
-        stage[rank][1] = make_float4(fmaf(J[19], J[20], J[22] * J[23]), fmaf(J[20], J[20], J[23] * J[23]),
-                                     fmaf(J[18], r0, J[21] * r1), fmaf(J[19], r0, J[22] * r1));
+        stage_a[rank] = make_float4(fmaf(J[18], J[18], J[21] * J[21]), fmaf(J[18], J[19], J[21] * J[22]),
+                                    fmaf(J[18], J[20], J[21] * J[23]), fmaf(J[19], J[19], J[22] * J[22]));
+        stage_b[rank] = make_float4(fmaf(J[19], J[20], J[22] * J[23]), fmaf(J[20], J[20], J[23] * J[23]),
+                                    fmaf(J[18], r0, J[21] * r1), fmaf(J[19], r0, J[22] * r1));
         stage_gz[rank] = fmaf(J[20], r0, J[23] * r1);
         __threadfence_block();
         const unsigned last = (unsigned)(re - rb - 1);
@@ -649,7 +655,7 @@ linearize_pipelined_kernel(View v, const float4* __restrict__ pts, const float* 
           float2 a0 = make_float2(0.f, 0.f), a1 = a0, b0 = a0, b1 = a0;
           float gz = 0.f;
           for (int r = rb; r < re; ++r) {  // rank order: V_k, g_p,k do not depend on the arrival order
-            const float4 x = stage[r][0], y = stage[r][1];
+            const float4 x = stage_a[r], y = stage_b[r];
             const float z = stage_gz[r];
             a0 = __fadd2_rn(a0, make_float2(x.x, x.y));
             a1 = __fadd2_rn(a1, make_float2(x.z, x.w));
@@ -1122,7 +1128,7 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   L.meta = up(L.vinv + max_pts * 48);  // V'^-1 in fp64, six entries per point
   L.stage_bytes = up(L.meta + meta_max);
   L.tbuf_bytes = up(3 * (T + 2) * 8);  // the point side is carried in fp64 (see schur_pass_kernel)
-  L.sbuf_bytes = up(3 * (T + 1) * 8);
+  L.sbuf_bytes = up(3 * (T + 5) * 8);
   const int hot_bytes = up(num_hot * 9 * 8);  // per-CTA fp64 accumulators of the hot cameras' q rows
   const int fixed = NG * (L.tbuf_bytes + L.sbuf_bytes) + NG * (T / 32) * kWarpScratchBytes + hot_bytes + 256;
   int st = (smem_limit - fixed) / L.stage_bytes;
@@ -1207,7 +1213,8 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   const int bar_id = 1 + g;
   // row stride T + 2: the six lanes of a point in phase B (component c, half h) read banks 2c + h + rank: distinct
   double(*tbuf)[T + 2] = reinterpret_cast<double(*)[T + 2]>(smem + L.tbuf + (size_t)g * L.tbuf_bytes);  // by rank
-  double(*sbuf)[T + 1] = reinterpret_cast<double(*)[T + 1]>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // by point
+  // row stride T + 5: the 15 storing lanes of phase B (point lp = 0..4, component c) hit 64-bit banks lp + 5 c: distinct
+  double(*sbuf)[T + 5] = reinterpret_cast<double(*)[T + 5]>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // by point
   float* rows = reinterpret_cast<float*>(smem + L.scratch + (size_t)(tid >> 5) * kWarpScratchBytes);
   int* camrow = reinterpret_cast<int*>(rows + 9 * 33);
   // p.q = sum_i u_i.e_i (+ p.lambda D_c p, added by the update kernel): the curvature of the operator AS COMPUTED,
@@ -1216,11 +1223,15 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   double dot_part = 0.0;
   int s = g % L.stages;  // stage of this group's current tile
   int round = g / L.stages;  // which fill of that stage it is
+  // With a stage count that is a multiple of NG every stage is always consumed by the same group, in program order:
+  // the parity wait alone is unambiguous and the `seen` guard (a shared-memory spin by all threads) is skipped.
+  const bool guard = (L.stages % NG) != 0;
   for (int t = blockIdx.x + g * G; t < v.num_tiles; t += NG * G) {
-    while (seen[s] < round) {
-    }
+    if (guard)
+      while (seen[s] < round) {
+      }
     mbar_wait(full + s, (unsigned)(round & 1));
-    if (gt == 0) seen[s] = round + 1;
+    if (guard && gt == 0) seen[s] = round + 1;
     const unsigned char* st = smem + (size_t)s * L.stage_bytes;
     const int npts = reinterpret_cast<const int*>(st + L.meta)[0];
     const unsigned short* pt_start = reinterpret_cast<const unsigned short*>(st + L.meta + 16);
