@@ -324,7 +324,7 @@ def make_scene(name: str, *, noise_free: bool = False, seed: Optional[int] = Non
 
     # --- measurements -------------------------------------------------------------------
     uv, depth = _project(cams_true.astype(np.float64), pts_true.astype(np.float64), cam_idx, pt_idx)
-    # visibility cull (reading C7: no depth guard in the model, so scenes keep P_z <= -5): drop the few
+    # visibility cull (reading G2; C7: no depth guard in the model, so scenes keep P_z <= -5): drop the few
     # grazing observations, never taking a point below two observations
     graze = depth > MAX_DEPTH
     if graze.any():
@@ -341,7 +341,7 @@ def make_scene(name: str, *, noise_free: bool = False, seed: Optional[int] = Non
     obs = uv.astype(np.float32)
 
     # --- perturbed start ----------------------------------------------------------------
-    # N(0, 0.01) on rotation / translation, applied in the camera's own frame (reading C16):
+    # N(0, 0.01) on rotation / translation, applied in the camera's own frame (reading G1):
     # R0 = Exp(d_w) R about the camera centre, C0 = C + d_c, t0 = -R0 C0.  Adding the noise to (w, t) of
     # P = R X + t literally would turn far cameras about the WORLD origin and throw their points by
     # |X| * 0.01 (up to ~8 units on the large grid), putting hundreds of observations behind the camera.
