@@ -153,6 +153,16 @@ int caspar_ba_solve(caspar_ba_t* h, int32_t iterations, float lambda0, float rel
  * next solve.  Errors: EINVAL. */
 int caspar_ba_set_preconditioner(caspar_ba_t* h, int32_t mode);
 
+/* PAPER.md:167-169 ("Separate kernels are used for the first iteration of the solver ... the initial score and the
+ * Jacobian are calculated simultaneously, while subsequent runs use the score values from the previous iteration") --
+ * the paper's fusion variant (N2).  mode 1: caspar_ba_lm_step evaluates the trial point x + delta with the
+ * FULL linearization kernel (residuals, Jacobians, V_k, g_p and the cost in one pass) into a second set of arrays
+ * (allocated here: 104 bytes per observation slot + 40 per point), and an accepted step swaps the two sets instead of
+ * linearizing again: the next caspar_ba_lm_step starts at S4 with the cost it already knows.  A rejected step throws
+ * the speculative Jacobians away.  Results are bit-identical to mode 0 (the same kernel at the same point).
+ * mode 0 (default): S9 is the residual-only pass.  Errors: EINVAL, ENOMEM. */
+int caspar_ba_set_fusion(caspar_ba_t* h, int32_t mode);
+
 /* PAPER.md:194-203 (residual only), :220 (fp32 summation is the paper's stated accuracy loss: the sum is fp64 here) --
  * step S9 without the update: F at the caller's current parameters.  cost_out: HOST, required. */
 int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out);
@@ -203,6 +213,9 @@ typedef struct {
   double reorder_seconds;    /* ... the S0 reordering (host, OpenMP)                                  */
   int32_t linearize_pipelined; /* 1: linearize and cost run as the persistent TMA-pipelined kernel      */
   int32_t reserved;
+  int64_t speculative_hits;    /* caspar_ba_set_fusion(1): accepted steps whose trial linearization was reused ... */
+  int64_t speculative_misses;  /* ... and rejected ones, whose trial linearization was thrown away                */
+  int64_t arena2_bytes;        /* second set of linearization arrays (0 until caspar_ba_set_fusion(h, 1))         */
 } caspar_ba_stats;
 /* Synchronises the stream the timed kernels ran on, then fills *out. */
 int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out);

@@ -25,6 +25,7 @@ EXPORTED_SYMBOLS = [
     "caspar_ba_export", "caspar_ba_schur_matvec", "caspar_ba_get_stats", "caspar_ba_set_profiling",
     "caspar_ba_last_error", "caspar_ba_layout_create", "caspar_ba_layout_get_info", "caspar_ba_layout_copy",
     "caspar_ba_layout_destroy", "caspar_ba_set_preconditioner", "caspar_ba_pcgnr_solve", "caspar_ba_set_linear_solver",
+    "caspar_ba_set_fusion",
 ]
 
 
@@ -54,7 +55,8 @@ class Stats(C.Structure):
                 ("matvec_pipelined", C.c_int32), ("pipeline_stages", C.c_int32),
                 ("num_hot_cameras", C.c_int32), ("device", C.c_int32),
                 ("create_seconds", C.c_double), ("reorder_seconds", C.c_double),
-                ("linearize_pipelined", C.c_int32), ("reserved", C.c_int32)]
+                ("linearize_pipelined", C.c_int32), ("reserved", C.c_int32),
+                ("speculative_hits", C.c_int64), ("speculative_misses", C.c_int64), ("arena2_bytes", C.c_int64)]
 
 
 class LayoutInfo(C.Structure):
@@ -126,6 +128,7 @@ def load_library() -> C.CDLL:
     L.caspar_ba_layout_destroy.argtypes = [vp]
     L.caspar_ba_layout_destroy.restype = None
     L.caspar_ba_set_preconditioner.argtypes = [vp, C.c_int32]
+    L.caspar_ba_set_fusion.argtypes = [vp, C.c_int32]
     L.caspar_ba_set_linear_solver.argtypes = [vp, C.c_int32]
     L.caspar_ba_pcgnr_solve.argtypes = [vp, C.c_float, C.c_float, C.c_int32, vp, C.POINTER(PcgInfo)]
     _lib = L
@@ -312,6 +315,9 @@ class CasparBA:
         st = Stats()
         self._check(self._lib.caspar_ba_get_stats(self._h, C.byref(st)), "get_stats")
         return st
+
+    def set_fusion(self, mode: int):
+        self._check(self._lib.caspar_ba_set_fusion(self._h, int(mode)), "set_fusion")
 
     def set_preconditioner(self, mode: int):
         self._check(self._lib.caspar_ba_set_preconditioner(self._h, int(mode)), "set_preconditioner")

@@ -50,8 +50,22 @@ struct caspar_ba {
   // no kernel argument changes between iterations (the iteration number is a device scalar), so the same graph
   // serves every chunk of every solve; captured once per handle on a private stream, launched on the caller's
   cudaStream_t capture_stream = nullptr;
-  cudaGraphExec_t chunk_graph = nullptr;
-  bool graph_tried = false;
+  cudaGraphExec_t chunk_graph[2] = {nullptr, nullptr};  // one per set of linearization arrays (see `alt`)
+  bool graph_tried[2] = {false, false};
+  // N2: a second set of the arrays a linearization writes.  With fusion on, S9 evaluates the trial
+  // point with the FULL linearize kernel into this set; an accepted step swaps the sets instead of linearizing again.
+  struct LinSet {
+    float4* J[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    float2* res = nullptr;
+    float4* V0 = nullptr;
+    float2* V1 = nullptr;
+    float4* gp = nullptr;
+  } alt;
+  void* arena2 = nullptr;  // holds `alt`; allocated by caspar_ba_set_fusion(h, 1)
+  size_t arena2_bytes = 0;
+  int fusion = 0;
+  int set_parity = 0;
+  long long speculative_hits = 0, speculative_misses = 0;
 };
 
 constexpr int kPcgChunk = 8;
@@ -271,10 +285,11 @@ int do_prepare(caspar_ba* h, double lambda, int preconditioner, cudaStream_t s) 
 
 // Capture one chunk of iterations.  Failure is not an error: the loop then launches the kernels one by one.
 static void build_chunk_graph(caspar_ba* h) {
-  h->graph_tried = true;
+  const int gp = h->set_parity;
+  h->graph_tried[gp] = true;
   if (const char* env = std::getenv("CASPAR_BA_GRAPH"))
     if (env[0] == '0') return;
-  if (cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking) != cudaSuccess) return;
+  if (!h->capture_stream && cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking) != cudaSuccess) return;
   cudaGraph_t graph = nullptr;
   bool ok = cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
   for (int i = 0; ok && i < kPcgChunk; ++i)
@@ -282,8 +297,8 @@ static void build_chunk_graph(caspar_ba* h) {
          launch_pcg_update(h->v, h->capture_stream) == cudaSuccess;
   const cudaError_t end = cudaStreamEndCapture(h->capture_stream, &graph);
   take_launch_count();  // captured launches are counted when the graph is launched
-  if (ok && end == cudaSuccess && graph && cudaGraphInstantiate(&h->chunk_graph, graph, 0) != cudaSuccess)
-    h->chunk_graph = nullptr;
+  if (ok && end == cudaSuccess && graph && cudaGraphInstantiate(&h->chunk_graph[gp], graph, 0) != cudaSuccess)
+    h->chunk_graph[gp] = nullptr;
   if (graph) cudaGraphDestroy(graph);
   cudaGetLastError();
 }
@@ -302,16 +317,17 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
   CK(launch_pcg_init(v, tol2, s));
   const int chunk = kPcgChunk;
   // whole chunks go out as one graph launch (not while per-launch profiling events are wanted)
-  if (!h->graph_tried && v.nc > 0 && v.num_tiles > 0) {
+  if (!h->graph_tried[h->set_parity] && v.nc > 0 && v.num_tiles > 0) {  // the kernel arguments hold the set's pointers
     account(h);
     build_chunk_graph(h);
   }
-  const bool use_graph = h->chunk_graph != nullptr && !h->profiling;
+  cudaGraphExec_t chunk_graph = h->chunk_graph[h->set_parity];
+  const bool use_graph = chunk_graph != nullptr && !h->profiling;
   int polled = 0;  // chunks whose flag copy has been enqueued
   bool stop = false;
   for (int it = 0; it < max_iter && !stop; ++it) {
     if (use_graph && it % chunk == 0 && it + chunk <= max_iter) {
-      CK(cudaGraphLaunch(h->chunk_graph, s));
+      CK(cudaGraphLaunch(chunk_graph, s));
       h->launches += 3ll * chunk;
       it += chunk - 1;
     } else {
@@ -557,7 +573,9 @@ void caspar_ba_destroy(caspar_ba_t* h) {
   for (cudaEvent_t e : h->ev_mv) cudaEventDestroy(e);
   for (cudaEvent_t e : h->poll_ev)
     if (e) cudaEventDestroy(e);
-  if (h->chunk_graph) cudaGraphExecDestroy(h->chunk_graph);
+  for (cudaGraphExec_t g : h->chunk_graph)
+    if (g) cudaGraphExecDestroy(g);
+  if (h->arena2) cudaFree(h->arena2);
   if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
   if (h->h_pcg) cudaFreeHost(h->h_pcg);
   if (h->h_step) cudaFreeHost(h->h_step);
@@ -653,7 +671,23 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   // trial point and its cost (S9)
   CK(launch_trial_update(v, s));
   CK(launch_camera_prepass(v, v.cams_trial, v.cam_table_trial, s));
-  CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
+  // N2: with fusion on, the trial point gets the FULL linearization (r, J, V, g_p and the cost in one pass) in the
+  // other set of arrays; if the step is accepted that IS the next iteration's linearization ("the
+  // initial score and the Jacobian are calculated simultaneously, while subsequent runs use the score values from the
+  // previous iteration").  (A forced rejection, accept_mode 2, speculates too: the tests use it for rejected steps.)
+  const bool speculate = h->fusion != 0 && h->arena2 != nullptr;
+  if (speculate) {
+    View w = v;
+    for (int i = 0; i < 6; ++i) w.J[i] = h->alt.J[i];
+    w.res = h->alt.res; w.V0 = h->alt.V0; w.V1 = h->alt.V1; w.gp = h->alt.gp;
+    {
+      Timed t(h, &h->ev_lin, s);
+      CK(launch_linearize_at(w, v.pts_trial, v.cam_table_trial, s));
+    }
+    CK(launch_linearize_cost(w, &v.step->trial_cost, s));
+  } else {
+    CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
+  }
   account(h);
   rc = sync_step_scalars(h, s);  // the one host synchronisation of the step
   if (rc) return rc;
@@ -695,10 +729,53 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   info->accepted = accept ? 1 : 0;
   if (accept) {
     CK(launch_commit(v, s));
-    account(h);
     h->linearized = false;
     h->prepared = false;
+    if (speculate && std::isfinite(info->cost_after)) {
+      // the trial linearization becomes the current one: swap the two sets, assemble the camera side (S4) from it
+      for (int i = 0; i < 6; ++i) std::swap(v.J[i], h->alt.J[i]);
+      std::swap(v.res, h->alt.res); std::swap(v.V0, h->alt.V0); std::swap(v.V1, h->alt.V1); std::swap(v.gp, h->alt.gp);
+      h->set_parity ^= 1;
+      CK(launch_assemble_cameras(v, s));
+      h->linearized = true;
+      h->have_delta = false;
+      h->cost = info->cost_after;
+      ++h->speculative_hits;
+    }
+    account(h);
+  } else if (speculate) {
+    ++h->speculative_misses;
   }
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_set_fusion(caspar_ba_t* h, int32_t mode) {
+  if (!h || (mode != 0 && mode != 1)) return CASPAR_BA_EINVAL;
+  DeviceGuard on_device(h->device);
+  if (mode == 1 && !h->arena2) {
+    const size_t S = (size_t)h->v.n_slots, NP = (size_t)h->v.np;
+    Carver sizer(nullptr);
+    auto lay = [&](Carver& c) {
+      for (int i = 0; i < 6; ++i) h->alt.J[i] = c.take<float4>(S);
+      h->alt.res = c.take<float2>(S);
+      h->alt.V0 = c.take<float4>(NP);
+      h->alt.V1 = c.take<float2>(NP);
+      h->alt.gp = c.take<float4>(NP);
+    };
+    lay(sizer);
+    h->arena2_bytes = (sizer.off + 255) & ~size_t(255);
+    cudaError_t e = cudaMalloc(&h->arena2, h->arena2_bytes);
+    if (e != cudaSuccess) {
+      h->arena2 = nullptr;
+      h->alt = caspar_ba::LinSet();
+      return fail(h, CASPAR_BA_ENOMEM, "second set of linearization arrays (" + std::to_string(h->arena2_bytes) + " bytes): " + cudaGetErrorString(e));
+    }
+    e = cudaMemset(h->arena2, 0, h->arena2_bytes);  // padding slots and unobserved points stay zero, as in the arena
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemset(arena2)");
+    Carver real(h->arena2);
+    lay(real);
+  }
+  h->fusion = mode;
   return CASPAR_BA_OK;
 }
 
@@ -827,6 +904,9 @@ int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {
   out->device = h->device;
   out->create_seconds = h->create_s;
   out->reorder_seconds = h->reorder_s;
+  out->speculative_hits = h->speculative_hits;
+  out->speculative_misses = h->speculative_misses;
+  out->arena2_bytes = (int64_t)h->arena2_bytes;
   return CASPAR_BA_OK;
 }
 

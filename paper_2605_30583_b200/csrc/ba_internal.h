@@ -182,6 +182,8 @@ cudaError_t launch_pack_points(const View& v, const float* points_caller, float4
 cudaError_t launch_unpack_points(const View& v, const float4* src, float* points_caller, cudaStream_t s);
 cudaError_t launch_camera_prepass(const View& v, const float* cams, float* table, cudaStream_t s);
 cudaError_t launch_linearize(const View& v, cudaStream_t s);
+// the same at another point: reads pts / table, writes the linearization arrays of `v` (N2: the trial point)
+cudaError_t launch_linearize_at(const View& v, const float4* pts, const float* table, cudaStream_t s);
 cudaError_t launch_linearize_cost(const View& v, double* cost_out, cudaStream_t s);  // folds launch_linearize's partials
 cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_out, cudaStream_t s);
 cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s);

@@ -2017,6 +2017,10 @@ static cudaError_t launch_reduce_cost(const View& v, bool pipelined, double* cos
 
 cudaError_t launch_linearize(const View& v, cudaStream_t s) { return launch_linearize_t<true>(v, v.pts, v.cam_table, s); }
 
+cudaError_t launch_linearize_at(const View& v, const float4* pts, const float* table, cudaStream_t s) {
+  return launch_linearize_t<true>(v, pts, table, s);
+}
+
 cudaError_t launch_linearize_cost(const View& v, double* cost_out, cudaStream_t s) {
   return launch_reduce_cost(v, linearize_pipelined(v), cost_out, s);
 }

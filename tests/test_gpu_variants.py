@@ -177,3 +177,68 @@ def test_lm_step_with_pcgnr(scene_cache, key):
     assert max(per_class_rel_l2(cams, o.cameras).values()) <= 1e-4
     g.close()
     o.close()
+
+
+# ------------------------------------------------------------------ N2: speculative trial linearization
+@pytest.mark.parametrize("key", list(SCENES))
+@pytest.mark.parametrize("camera_model", [0, 1])
+def test_fused_trial_linearization_matches_the_default_path(scene_cache, key, camera_model):
+    """caspar_ba_set_fusion(1): S9 runs the FULL linearize kernel at the trial point into a second
+    set of arrays and an accepted step swaps the sets instead of linearizing again.  The same kernel at the same
+    point, so the two paths differ only by what two runs of ONE path differ by: the order of the fp64 REDs inside
+    the Schur matvec (C14, ~1e-16 per solve).  A fixed schedule of forced accepts and rejects at lambda = 1e-2
+    (rejected steps throw the speculative Jacobians away and solve again from the kept linearization): step records
+    to 1e-7, parameters and the linearization left behind to 1e-5."""
+    name, kw = SCENES[key]
+    s = scene_cache(name, **kw)
+    decisions = [1, 1, 2, 1, 2, 2, 1, 1]
+    runs = []
+    for fusion in (0, 1):
+        g = pkg.CasparBA.from_scene(s, camera_model=camera_model)
+        g.set_fusion(fusion)
+        # ten PCG iterations, no tolerance: a long unconverged CG run amplifies the last-bit differences of the RED order
+        steps = [g.lm_step(LAM * 0.5 ** t, 0.0, 10, mode) for t, mode in enumerate(decisions)]
+        stats = g.stats()
+        if fusion == 0:      # the linearization the next step would start from
+            g.linearize()
+        arrays = [g.export(w) for w in (pkg.RESIDUALS, pkg.JC, pkg.JP, pkg.U, pkg.V, pkg.G)]
+        runs.append((steps, g.cameras.cpu().numpy(), g.points.cpu().numpy(), arrays, stats))
+        g.close()
+    (s0, c0, p0, a0, st0), (s1, c1, p1, a1, st1) = runs
+    for x, y, mode in zip(s0, s1, decisions):
+        assert x.accepted == y.accepted == (mode == 1) and x.pcg_iterations == y.pcg_iterations
+        assert x.cost_before == pytest.approx(y.cost_before, rel=1e-7)
+        assert x.cost_after == pytest.approx(y.cost_after, rel=1e-7)
+        if x.model_decrease > 1e-6 * x.cost_before:
+            assert x.model_decrease == pytest.approx(y.model_decrease, rel=1e-4)
+    assert np.abs(c0 - c1).max() <= 1e-5 * np.abs(c0).max() and np.abs(p0 - p1).max() <= 1e-5 * np.abs(p0).max()
+    assert st0.speculative_hits == 0 and st0.speculative_misses == 0 and st0.arena2_bytes == 0
+    assert st1.speculative_hits == decisions.count(1) and st1.speculative_misses == decisions.count(2)
+    assert st1.arena2_bytes > 0
+    for x, y in zip(a0, a1):  # the fused run already holds the linearization at the new point
+        assert rel_l2(x, y) <= 1e-5
+
+
+def test_fusion_survives_a_parameter_reset_and_the_graph_chunks(scene_cache):
+    """After set_parameters_host the speculative linearization is stale and must not be used; the CUDA-graph PCG
+    chunks hold the pointers of ONE set of Jacobians, so both sets need their own graph."""
+    import torch
+    s = scene_cache("small")
+    g = pkg.CasparBA.from_scene(s)
+    g.set_fusion(1)
+    ref = pkg.CasparBA.from_scene(s)
+    a = [g.lm_step(LAM, 1e-6, s.pcg_max_iter, 0) for _ in range(3)]       # three accepted steps: sets swap 3 times
+    b = [ref.lm_step(LAM, 1e-6, s.pcg_max_iter, 0) for _ in range(3)]
+    for x, y in zip(a, b):
+        assert x.accepted and y.accepted and x.pcg_iterations == y.pcg_iterations
+        assert x.cost_after == pytest.approx(y.cost_after, rel=1e-7)
+    cam_h = torch.from_numpy(s.cameras.copy()).pin_memory()
+    pts_h = torch.from_numpy(s.points.copy()).pin_memory()
+    g.set_parameters_host(cam_h, pts_h)
+    ref.set_parameters_host(cam_h, pts_h)
+    x, y = g.lm_step(LAM, 1e-6, s.pcg_max_iter, 0), ref.lm_step(LAM, 1e-6, s.pcg_max_iter, 0)
+    assert x.pcg_iterations == y.pcg_iterations
+    assert x.cost_before == pytest.approx(y.cost_before, rel=1e-12) and x.cost_after == pytest.approx(y.cost_after, rel=1e-7)
+    assert x.cost_before == pytest.approx(b[0].cost_before, rel=1e-12)
+    g.close()
+    ref.close()
