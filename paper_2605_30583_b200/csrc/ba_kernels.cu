@@ -1108,7 +1108,7 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
 // long-scoreboard stalls at 39 % of HBM peak (history).
 // ------------------------------------------------------------------------------------------------
 struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
-  int j, cam, rank, vinv, meta, stage_bytes;
+  int j, cam, rank, vinv, gp, meta, stage_bytes;
   int stages, groups, tbuf, tbuf_bytes, sbuf, sbuf_bytes, scratch, hot, bars, total;
 };
 
@@ -1116,8 +1116,9 @@ constexpr int kWarpScratchBytes = 1408;  // per consumer warp: 9 x 33 floats of 
 
 // NG consumer groups of T threads share the ring; each group owns a staging area for the point-side sums
 // t_k (by rank) and one for the per-point results s_k (by local point id).
+// with_gp: the stage also carries the tile's g_p rows (the S5 / S8 instantiations of the kernel)
 __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, int meta_max, int num_hot,
-                                                  int smem_limit) {
+                                                  int smem_limit, bool with_gp = false) {
   PipeLayout L;
   auto up = [](int x) { return (x + 127) & ~127; };
   L.groups = NG;
@@ -1125,7 +1126,8 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   L.cam = L.j + 6 * T * 16;
   L.rank = L.cam + T * 4;
   L.vinv = up(L.rank + T * 2);
-  L.meta = up(L.vinv + max_pts * 48);  // V'^-1 in fp64, six entries per point
+  L.gp = up(L.vinv + max_pts * 48);  // V'^-1 in fp64, six entries per point
+  L.meta = with_gp ? up(L.gp + max_pts * 16) : L.gp;
   L.stage_bytes = up(L.meta + meta_max);
   L.tbuf_bytes = up(3 * (T + 2) * 8);  // the point side is carried in fp64 (see schur_pass_kernel)
   L.sbuf_bytes = up(3 * (T + 5) * 8);
@@ -1143,10 +1145,12 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
 }
 
 
-template <int T, int NG, bool HOT>
+// MODE = MATVEC (S6), RHS (S5) or BACKSUB (S8): the same pass as schur_pass_kernel, see there.  RHS and BACKSUB also
+// stream the tile's g_p rows into the stage; BACKSUB has no camera side (HOT is false there).
+template <int T, int NG, bool HOT, int MODE>
 __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(View v, PipeLayout L) {
   extern __shared__ __align__(128) unsigned char smem[];
-  if (v.pcg->done) return;
+  if (MODE == MATVEC && v.pcg->done) return;
   const int tid = threadIdx.x;
   unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L.bars);
   unsigned long long* empty = full + kMaxStages;
@@ -1167,7 +1171,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       seen[s] = 0;
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    if (blockIdx.x == 0) {  // accumulators of the update that follows this matvec
+    if (MODE == MATVEC && blockIdx.x == 0) {  // accumulators of the update that follows this matvec
       const int nxt = (v.pcg->it_a + 1) & 1;  // it_a: written by the previous update kernel only
       v.pcg->rz[nxt] = 0.0;
       v.pcg->pDp[nxt] = 0.0;
@@ -1193,13 +1197,15 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         mbar_wait(empty + s, ph ^ 1);
         unsigned char* st = smem + (size_t)s * L.stage_bytes;
         const unsigned vinv_bytes = (unsigned)d.w * 48u;
-        mbar_expect_tx(full + s, (unsigned)(6 * T * 16 + T * 4 + T * 2) + vinv_bytes + (unsigned)d.y);
+        const unsigned gp_bytes = MODE == MATVEC ? 0u : (unsigned)d.w * 16u;
+        mbar_expect_tx(full + s, (unsigned)(6 * T * 16 + T * 4 + T * 2) + vinv_bytes + gp_bytes + (unsigned)d.y);
         const long long slot0 = (long long)t * T;
 #pragma unroll
         for (int c = 0; c < 6; ++c) bulk_g2s(st + L.j + c * T * 16, v.J[c] + slot0, T * 16, full + s, pol_stream);
         bulk_g2s(st + L.cam, v.cam + slot0, T * 4, full + s, pol_stream);
         bulk_g2s(st + L.rank, v.rankpid + slot0, T * 2, full + s, pol_stream);
         bulk_g2s(st + L.vinv, v.Vinv64 + 6ll * d.z, vinv_bytes, full + s, pol_keep);
+        if (MODE != MATVEC) bulk_g2s(st + L.gp, v.gp + d.z, gp_bytes, full + s, pol_stream);
         bulk_g2s(st + L.meta, v.tile_meta + 16ll * d.x, (unsigned)d.y, full + s, pol_stream);
         d = dn;
         if (++s == L.stages) { s = 0; ph ^= 1; }
@@ -1221,6 +1227,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   // which is what keeps alpha consistent with q (a rewritten, manifestly positive form was tried and made CG
   // diverge at lambda ~ 1e-5: DESIGN.md "PCG at tiny lambda").  fp64 accumulation.
   double dot_part = 0.0;
+  double dg_part = 0.0;  // BACKSUB: delta_p . g_p
   int s = g % L.stages;  // stage of this group's current tile
   int round = g / L.stages;  // which fill of that stage it is
   // With a stage count that is a multiple of NG every stage is always consumed by the same group, in program order:
@@ -1240,7 +1247,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     const unsigned rank = rp & 255u, pid = rp >> 8;
     // ---- phase A: u = J_c p_j, scatter J_p^T u to the point-major staging rows
     float4 pa = make_float4(0.f, 0.f, 0.f, 0.f), pb = pa, pc = pa;
-    if (cam >= 0) {
+    if (MODE != RHS && cam >= 0) {  // p_j (MATVEC) or delta_c,j (BACKSUB); RHS has no camera vector: u = 0
       const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
       pa = __ldg(pv); pb = __ldg(pv + 1); pc = __ldg(pv + 2);
     }
@@ -1269,7 +1276,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       }
 #pragma unroll
       for (int k = 0; k < 18; ++k) Jc[k] = J[k];
-      if (cam >= 0) {
+      if (MODE != RHS && cam >= 0) {
         const double u0 = (double)uf0, u1 = (double)uf1;
         tbuf[0][rank] = fma((double)J[18], u0, (double)J[21] * u1);
         tbuf[1][rank] = fma((double)J[19], u0, (double)J[22] * u1);
@@ -1286,12 +1293,18 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         const bool valid = lane < 30 && k < npts;
         const int rb = valid ? pt_start[k] : 0, re = valid ? pt_start[k + 1] : 0;
         double tsum = 0.0;
-        for (int r = rb + half; r < re; r += 8) {  // four independent loads per round
-          const double a0 = tbuf[c][r];
-          const double a1 = r + 2 < re ? tbuf[c][r + 2] : 0.0;
-          const double a2 = r + 4 < re ? tbuf[c][r + 4] : 0.0;
-          const double a3 = r + 6 < re ? tbuf[c][r + 6] : 0.0;
-          tsum += (a0 + a1) + (a2 + a3);
+        if (MODE != RHS)
+          for (int r = rb + half; r < re; r += 8) {  // four independent loads per round
+            const double a0 = tbuf[c][r];
+            const double a1 = r + 2 < re ? tbuf[c][r + 2] : 0.0;
+            const double a2 = r + 4 < re ? tbuf[c][r + 4] : 0.0;
+            const double a3 = r + 6 < re ? tbuf[c][r + 6] : 0.0;
+            tsum += (a0 + a1) + (a2 + a3);
+          }
+        double gc = 0.0;  // component c of g_p,k (RHS: t = g_p; BACKSUB: t = sum + g_p)
+        if (MODE != MATVEC && valid && half == 0) {
+          gc = (double)reinterpret_cast<const float*>(st + L.gp)[4 * k + c];
+          tsum += gc;
         }
         tsum += __shfl_xor_sync(0xffffffffu, tsum, 1);
         const int base = 6 * lp;
@@ -1301,7 +1314,13 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
           const double* vi = reinterpret_cast<const double*>(st + L.vinv) + 6 * k;  // xx xy xz yy yz zz
           // row c of the symmetric 3x3: (0: xx xy xz) (1: xy yy yz) (2: xz yz zz)
           const double m0 = vi[c], m1 = vi[c == 0 ? 1 : (c == 1 ? 3 : 4)], m2 = vi[c == 0 ? 2 : (c == 1 ? 4 : 5)];
-          sbuf[c][k] = m0 * t0 + m1 * t1 + m2 * t2;
+          double sc = m0 * t0 + m1 * t1 + m2 * t2;
+          if (MODE == BACKSUB) {  // delta_p,k = -V'^-1 (g_p,k + sum J_p^T J_c delta_c); delta_p.g_p for the gain ratio
+            sc = -sc;
+            reinterpret_cast<float*>(v.dp + reinterpret_cast<const int*>(st + L.meta)[3] + k)[c] = (float)sc;
+            dg_part += sc * gc;
+          }
+          sbuf[c][k] = sc;
         }
       }
     }
@@ -1315,15 +1334,28 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         const float4 x5 = reinterpret_cast<const float4*>(st + L.j + 5 * T * 16)[gt];  // Jp2 .. Jp5
         const double u0 = (double)uf0, u1 = (double)uf1;
         const double s0 = sbuf[0][pid], s1 = sbuf[1][pid], s2 = sbuf[2][pid];
-        const double ed0 = u0 - ((double)x4.z * s0 + (double)x4.w * s1 + (double)x5.x * s2);
-        const double ed1 = u1 - ((double)x5.y * s0 + (double)x5.z * s1 + (double)x5.w * s2);
-        dot_part += u0 * ed0 + u1 * ed1;
-        e0 = (float)ed0;
-        e1 = (float)ed1;
+        const double w0 = (double)x4.z * s0 + (double)x4.w * s1 + (double)x5.x * s2;  // J_p s_k
+        const double w1 = (double)x5.y * s0 + (double)x5.z * s1 + (double)x5.w * s2;
+        if (MODE == BACKSUB) {  // |J delta|^2 of this observation
+          const double y0 = u0 + w0, y1 = u1 + w1;
+          dot_part += y0 * y0 + y1 * y1;
+        } else {
+          const double ed0 = MODE == MATVEC ? u0 - w0 : w0, ed1 = MODE == MATVEC ? u1 - w1 : w1;
+          if (MODE == MATVEC) dot_part += u0 * ed0 + u1 * ed1;
+          e0 = (float)ed0;
+          e1 = (float)ed1;
+        }
       }
+      if (MODE != BACKSUB) {
 #pragma unroll
-      for (int k = 0; k < 9; ++k) c9[k] = fmaf(Jc[k], e0, Jc[9 + k] * e1);
+        for (int k = 0; k < 9; ++k) c9[k] = fmaf(Jc[k], e0, Jc[9 + k] * e1);
+      }
     }
+    if (MODE == BACKSUB) {  // no camera side: the stage reads above feed registers only, so fence them (section 5.2)
+      fence_reads_before_refill();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + s);
+    } else
     // ---- camera side, warp-local.  The tile's slots are sorted by camera, so a warp holds whole pieces of
     // camera runs (lane intervals).  The nine products go to the warp's scratch rows (bank = component + lane:
     // conflict free); lane (k, part) then walks component k over slots [11 part, 11 part + 11) and adds a
@@ -1354,7 +1386,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
 #pragma unroll
         for (int i = 0; i < 11; ++i) val[i] = (i < 10 || part < 2) ? src[i] : 0.f;
         float acc = 0.f;
-        double* qk = v.q + k;
+        double* qk = (MODE == MATVEC ? v.q : v.b) + k;
 #pragma unroll
         for (int i = 0; i < 11; ++i) {
           acc += val[i];
@@ -1374,22 +1406,43 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     s += NG;
     while (s >= L.stages) { s -= L.stages; ++round; }
   }
-  // p.q: one fp64 atomic per CTA (same-address atomics serialise in L2: 3,552 per-warp ones would trail the kernel)
-  const double tot = warp_sum(dot_part);
-  double* warp_tot = reinterpret_cast<double*>(rows);  // this warp's scratch row is free now
-  if (lane == 0) warp_tot[0] = tot;
-  group_bar(15, NG * T);  // all consumer groups are done
-  if (tid < 32) {
-    double a = 0.0;
-    for (int w = lane; w < NG * (T / 32); w += 32)
-      a += *reinterpret_cast<const double*>(smem + L.scratch + (size_t)w * kWarpScratchBytes);
-    a = warp_sum(a);
-    if (lane == 0) atomicAdd(&v.pcg->pq, a);
+  // p.q (MATVEC) / |J delta|^2 and delta_p.g_p (BACKSUB): one fp64 atomic per CTA (same-address atomics serialise in
+  // L2: 3,552 per-warp ones would trail the kernel)
+  if (MODE != RHS) {
+    const double tot = warp_sum(dot_part);
+    const double tot2 = MODE == BACKSUB ? warp_sum(dg_part) : 0.0;
+    double* warp_tot = reinterpret_cast<double*>(rows);  // this warp's scratch row is free now
+    if (lane == 0) {
+      warp_tot[0] = tot;
+      warp_tot[1] = tot2;
+    }
+    group_bar(15, NG * T);  // all consumer groups are done
+    if (tid < 32) {
+      double a = 0.0, b = 0.0;
+      for (int w = lane; w < NG * (T / 32); w += 32) {
+        const double* wt = reinterpret_cast<const double*>(smem + L.scratch + (size_t)w * kWarpScratchBytes);
+        a += wt[0];
+        b += wt[1];
+      }
+      a = warp_sum(a);
+      if (MODE == BACKSUB) b = warp_sum(b);
+      if (lane == 0) {
+        if (MODE == MATVEC) {
+          atomicAdd(&v.pcg->pq, a);
+        } else {
+          atomicAdd(&v.step->jd2, a);
+          atomicAdd(&v.step->dg, b);
+        }
+      }
+    }
+  } else if (HOT) {
+    group_bar(15, NG * T);  // the hot accumulators below are complete once every group is done
   }
   if (HOT) {  // one RED per hot camera row and CTA
+    double* dst = MODE == MATVEC ? v.q : v.b;
     for (int i = tid; i < 9 * v.num_hot; i += NG * T) {
       const double a = hot_acc[i];
-      if (a != 0.0) atomicAdd(v.q + 9ll * __ldg(v.hot_list + i / 9) + i % 9, a);
+      if (a != 0.0) atomicAdd(dst + 9ll * __ldg(v.hot_list + i / 9) + i % 9, a);
     }
   }
 }
@@ -2078,7 +2131,6 @@ static cudaError_t launch_pass(const View& v, cudaStream_t s) {
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pass<RHS>(v, s); }
 
 // The pipelined matvec needs the opt-in shared-memory limit and at least two stages; otherwise (or with
 // CASPAR_BA_PIPELINE=0) the one-block-per-tile kernel is used.
@@ -2111,8 +2163,14 @@ int pipeline_stages(const View& v) {
 // handles with different layouts share the kernel.
 template <int T, int NG>
 static cudaError_t pipelined_attr(bool hot) {
-  return hot ? cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin())
-             : cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin());
+  const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  cudaError_t e = hot ? cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, true, MATVEC>, attr, smem_optin())
+                      : cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, false, MATVEC>, attr, smem_optin());
+  if (e == cudaSuccess)
+    e = hot ? cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, true, RHS>, attr, smem_optin())
+            : cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, false, RHS>, attr, smem_optin());
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(schur_matvec_pipelined_kernel<T, NG, false, BACKSUB>, attr, smem_optin());
+  return e;
 }
 
 template <int T, int NG>
@@ -2137,23 +2195,30 @@ cudaError_t configure_kernels(const View& v) {
   return pipelined_attr<128, 6>(hot);
 }
 
-template <int T, int NG>
+template <int T, int NG, int MODE>
 static void pipelined_launch(const View& v, const PipeLayout& L, int grid, cudaStream_t s) {
-  if (v.num_hot > 0)
-    schur_matvec_pipelined_kernel<T, NG, true><<<grid, NG * T + 32, L.total, s>>>(v, L);
+  if (MODE != BACKSUB && v.num_hot > 0)
+    schur_matvec_pipelined_kernel<T, NG, MODE != BACKSUB, MODE><<<grid, NG * T + 32, L.total, s>>>(v, L);
   else
-    schur_matvec_pipelined_kernel<T, NG, false><<<grid, NG * T + 32, L.total, s>>>(v, L);
+    schur_matvec_pipelined_kernel<T, NG, false, MODE><<<grid, NG * T + 32, L.total, s>>>(v, L);
 }
 
-cudaError_t launch_schur_matvec(const View& v, cudaStream_t s) {
-  if (!pipelined_matvec_available(v)) return launch_pass<MATVEC>(v, s);
-  const PipeLayout L = pipe_layout(v.T, pipe_groups(v.T), v.max_pts_per_tile, v.meta_max_bytes, v.num_hot, smem_optin());
+// S5 / S6 / S8 through the persistent TMA-pipelined kernel when the handle uses it (and, for S5 / S8, whose stages also
+// carry the g_p rows, the ring still has a stage to spare), else through the one-block-per-tile pass.
+template <int MODE>
+static cudaError_t launch_pipelined_or_pass(const View& v, cudaStream_t s) {
+  if (!pipelined_matvec_available(v)) return launch_pass<MODE>(v, s);
+  const int NG = pipe_groups(v.T);
+  const PipeLayout L = pipe_layout(v.T, NG, v.max_pts_per_tile, v.meta_max_bytes, v.num_hot, smem_optin(), MODE != MATVEC);
+  if (L.stages < NG + 1) return launch_pass<MODE>(v, s);
   const int grid = v.num_tiles < v.num_sms ? v.num_tiles : v.num_sms;
-  if (v.T == 256) pipelined_launch<256, 3>(v, L, grid, s);
-  else if (v.T == 192) pipelined_launch<192, 4>(v, L, grid, s);
-  else pipelined_launch<128, 6>(v, L, grid, s);
+  if (v.T == 256) pipelined_launch<256, 3, MODE>(v, L, grid, s);
+  else if (v.T == 192) pipelined_launch<192, 4, MODE>(v, L, grid, s);
+  else pipelined_launch<128, 6, MODE>(v, L, grid, s);
   return CBA_LAUNCHED();
 }
+
+cudaError_t launch_schur_matvec(const View& v, cudaStream_t s) { return launch_pipelined_or_pass<MATVEC>(v, s); }
 
 cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s) {
   if (v.nc == 0) return cudaSuccess;
@@ -2181,8 +2246,10 @@ cudaError_t launch_backsub(const View& v, cudaStream_t s) {
     e = CBA_LAUNCHED();
   }
   if (e != cudaSuccess) return e;
-  return launch_pass<BACKSUB>(v, s);
+  return launch_pipelined_or_pass<BACKSUB>(v, s);
 }
+
+cudaError_t launch_schur_rhs(const View& v, cudaStream_t s) { return launch_pipelined_or_pass<RHS>(v, s); }
 
 template <bool FINAL>
 static cudaError_t launch_full_pass(const View& v, cudaStream_t s) {
