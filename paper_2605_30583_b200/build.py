@@ -53,9 +53,47 @@ def ptxas_table() -> str:
     return "\n".join(rows)
 
 
+def sass_evidence() -> str:
+    """The instructions that prove the TMA / mbarrier path in the built library's two persistent kernels
+    (`python -m paper_2605_30583_b200.build --sass-evidence`): UBLKCP (cp.async.bulk), SYNCS (mbarrier),
+    FENCE.VIEW.ASYNC (fence.proxy.async), RED / ATOM, with their counts and the first occurrence of each in context."""
+    import collections
+    import re
+
+    build()
+    names = subprocess.run(["cuobjdump", "-sass", LIBRARY], capture_output=True, text=True, check=True).stdout
+    out = []
+    for kernel in ("schur_matvec_pipelined_kernelILi256ELi3ELb0ELi0E", "linearize_pipelined_kernelILi256ELi3ELb1E"):
+        m = re.search(r"Function : (\S*%s\S*)" % kernel, names)
+        if not m:
+            continue
+        fn = m.group(1)
+        sass = subprocess.run(["cuobjdump", "-sass", "-fun", fn, LIBRARY], capture_output=True, text=True).stdout
+        lines = [re.sub(r"\s*/\* 0x[0-9a-f]+ \*/\s*$", "", ln) for ln in sass.splitlines() if re.search(r"/\*[0-9a-f]{4}\*/", ln)]
+        demangled = subprocess.run(["c++filt", fn], capture_output=True, text=True).stdout.strip()
+        out.append(f"## `{demangled}` ({len(lines)} SASS instructions)\n")
+        counts = collections.Counter()
+        first = {}
+        pat = re.compile(r"\b(UBLKCP\S*|SYNCS\.\S+|FENCE\.VIEW\.ASYNC\S*|REDG?\.\S+|ATOM[SG]?\.\S+|BAR\.\S+|MEMBAR\.\S+)")
+        for i, ln in enumerate(lines):
+            mm = pat.search(ln)
+            if mm:
+                counts[mm.group(1)] += 1
+                first.setdefault(mm.group(1), i)
+        out.append("| mnemonic | count |\n|---|---|")
+        out += [f"| `{k}` | {v} |" for k, v in sorted(counts.items())]
+        out.append("\nFirst occurrence of each, with the two instructions before and after:\n\n```")
+        for k, i in sorted(first.items(), key=lambda x: x[1]):
+            out += [ln.strip() for ln in lines[max(0, i - 2):i + 3]] + ["..."]
+        out.append("```\n")
+    return "\n".join(out)
+
+
 if __name__ == "__main__":
     import sys
-    if "--ptxas-table" in sys.argv:
+    if "--sass-evidence" in sys.argv:
+        print(sass_evidence())
+    elif "--ptxas-table" in sys.argv:
         print(ptxas_table())
     else:
         print(build(force=True, verbose="-v" in sys.argv))
