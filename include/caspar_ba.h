@@ -163,6 +163,26 @@ int caspar_ba_set_preconditioner(caspar_ba_t* h, int32_t mode);
  * mode 0 (default): S9 is the residual-only pass.  Errors: EINVAL, ENOMEM. */
 int caspar_ba_set_fusion(caspar_ba_t* h, int32_t mode);
 
+/* SURVEY.md 8(e) (the paper itself is single-GPU; its "shared add", taken across devices) --
+ * POINT-SHARDED problem: the handle is ONE SHARD.  It was created with ALL cameras (replicated on every shard, the
+ * same values) and a SUBSET of the points with all their observations (point ids local to the shard).  Every partial
+ * sum over observations is then summed over the shards before it is used, through the caller's collective:
+ *   fn(ctx, count, op, cuda_stream)  op 0: sum the first `count` DOUBLES of the exchange buffer over all shards, in
+ *                                          place, result on every shard (an all-reduce);
+ *                                    op 1: replace the first `count` BYTES of the buffer by the ROOT shard's
+ *                                          (a broadcast);  both enqueued on `cuda_stream`; return 0 on success.
+ * exchange_buffer_dev: DEVICE, caller-owned, >= 54 * num_cameras + 8 doubles, borrowed until the next
+ * caspar_ba_set_shard / destroy.  is_root: exactly one shard passes 1 (it contributes the replicated camera terms).
+ * Exchanges per call: linearize 1 (U, g_c, cost); pcg_solve 1 (+1 with the Schur-Jacobi preconditioner) + 3 for the
+ * right-hand side and the start + 3 per iteration (q and p.q summed; the root's PCG scalars broadcast after each of
+ * the two update kernels so that alpha, beta, the direction scale and the stop decision are bit-identical on every
+ * shard) + 1; lm_step adds 1 (trial cost, |J delta|^2, delta.g).  All shards must make the same calls in the same
+ * order.  The CUDA-graph PCG chunks, caspar_ba_set_fusion and caspar_ba_pcgnr_solve are not used on a sharded handle.
+ * fn = NULL returns the handle to a single-GPU problem.  Errors: EINVAL (buffer too small). */
+typedef int (*caspar_ba_exchange_fn)(void* ctx, size_t count, int32_t op, void* cuda_stream);
+int caspar_ba_set_shard(caspar_ba_t* h, caspar_ba_exchange_fn fn, void* ctx, double* exchange_buffer_dev,
+                        size_t exchange_count, int32_t is_root);
+
 /* PAPER.md:194-203 (residual only), :220 (fp32 summation is the paper's stated accuracy loss: the sum is fp64 here) --
  * step S9 without the update: F at the caller's current parameters.  cost_out: HOST, required. */
 int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out);
@@ -216,6 +236,7 @@ typedef struct {
   int64_t speculative_hits;    /* caspar_ba_set_fusion(1): accepted steps whose trial linearization was reused ... */
   int64_t speculative_misses;  /* ... and rejected ones, whose trial linearization was thrown away                */
   int64_t arena2_bytes;        /* second set of linearization arrays (0 until caspar_ba_set_fusion(h, 1))         */
+  int64_t shard_exchanges;     /* calls of the caspar_ba_set_shard collective so far                               */
 } caspar_ba_stats;
 /* Synchronises the stream the timed kernels ran on, then fills *out. */
 int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out);

@@ -8,3 +8,5 @@ point-eliminated (Schur) normal equations.  The product is the C-ABI library
 from .binding import (CasparBA, CasparError, PcgInfo, Stats, Step, StepInfo, EXPORTED_SYMBOLS,  # noqa: F401
                       load_library, library_path, plan_layout)
 from .binding import RESIDUALS, JC, JP, U, V, G, SCHUR_RHS, DELTA, PRECONDITIONER  # noqa: F401
+from .binding import OK, EINVAL, ECUDA, ENOMEM, ENUMERIC, ESTATE  # noqa: F401
+from . import sharding  # noqa: F401

@@ -25,7 +25,7 @@ EXPORTED_SYMBOLS = [
     "caspar_ba_export", "caspar_ba_schur_matvec", "caspar_ba_get_stats", "caspar_ba_set_profiling",
     "caspar_ba_last_error", "caspar_ba_layout_create", "caspar_ba_layout_get_info", "caspar_ba_layout_copy",
     "caspar_ba_layout_destroy", "caspar_ba_set_preconditioner", "caspar_ba_pcgnr_solve", "caspar_ba_set_linear_solver",
-    "caspar_ba_set_fusion",
+    "caspar_ba_set_fusion", "caspar_ba_set_shard",
 ]
 
 
@@ -56,7 +56,12 @@ class Stats(C.Structure):
                 ("num_hot_cameras", C.c_int32), ("device", C.c_int32),
                 ("create_seconds", C.c_double), ("reorder_seconds", C.c_double),
                 ("linearize_pipelined", C.c_int32), ("reserved", C.c_int32),
-                ("speculative_hits", C.c_int64), ("speculative_misses", C.c_int64), ("arena2_bytes", C.c_int64)]
+                ("speculative_hits", C.c_int64), ("speculative_misses", C.c_int64), ("arena2_bytes", C.c_int64),
+                ("shard_exchanges", C.c_int64)]
+
+
+# int fn(void* ctx, size_t count, int32_t op, void* cuda_stream)
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_size_t, C.c_int32, C.c_void_p)
 
 
 class LayoutInfo(C.Structure):
@@ -129,6 +134,7 @@ def load_library() -> C.CDLL:
     L.caspar_ba_layout_destroy.restype = None
     L.caspar_ba_set_preconditioner.argtypes = [vp, C.c_int32]
     L.caspar_ba_set_fusion.argtypes = [vp, C.c_int32]
+    L.caspar_ba_set_shard.argtypes = [vp, EXCHANGE_FN, vp, vp, C.c_size_t, C.c_int32]
     L.caspar_ba_set_linear_solver.argtypes = [vp, C.c_int32]
     L.caspar_ba_pcgnr_solve.argtypes = [vp, C.c_float, C.c_float, C.c_int32, vp, C.POINTER(PcgInfo)]
     _lib = L
@@ -315,6 +321,31 @@ class CasparBA:
         st = Stats()
         self._check(self._lib.caspar_ba_get_stats(self._h, C.byref(st)), "get_stats")
         return st
+
+    def set_shard(self, exchange, is_root: bool):
+        """Make this handle ONE SHARD of a point-sharded problem (include/caspar_ba.h: caspar_ba_set_shard).
+        `exchange(buffer, count, op)` is called with the handle's exchange buffer (a float64 CUDA tensor), on the
+        current stream: op 0 sums buffer[:count] over the shards in place, op 1 replaces the first `count` BYTES by the
+        root shard's.  `exchange=None` returns to a single-GPU problem.  See `sharding.torch_exchange`."""
+        if exchange is None:
+            self._check(self._lib.caspar_ba_set_shard(self._h, EXCHANGE_FN(0), None, None, 0, 1), "set_shard")
+            self._exchange_cb = self._xchg = None
+            return
+        self._xchg = torch.zeros(54 * self.nc + 8, dtype=torch.float64, device=self.device)
+        buf = self._xchg
+
+        def _cb(_ctx, count, op, _stream):
+            try:
+                exchange(buf, int(count), int(op))
+                return 0
+            except Exception:  # never let an exception cross the C ABI
+                import traceback
+                traceback.print_exc()
+                return 1
+
+        self._exchange_cb = EXCHANGE_FN(_cb)      # keep the trampoline alive as long as the handle uses it
+        self._check(self._lib.caspar_ba_set_shard(self._h, self._exchange_cb, None, buf.data_ptr(), buf.numel(),
+                                                  1 if is_root else 0), "set_shard")
 
     def set_fusion(self, mode: int):
         self._check(self._lib.caspar_ba_set_fusion(self._h, int(mode)), "set_fusion")

@@ -65,6 +65,12 @@ struct caspar_ba {
   size_t arena2_bytes = 0;
   int fusion = 0;
   int set_parity = 0;
+  // point-sharded problem: this handle is one shard; `exchange` sums / broadcasts over the shards
+  caspar_ba_exchange_fn exchange = nullptr;
+  void* exchange_ctx = nullptr;
+  double* xchg = nullptr;      // DEVICE exchange buffer (caller's), xchg_count doubles
+  size_t xchg_count = 0;
+  long long exchanges = 0;
   long long speculative_hits = 0, speculative_misses = 0;
 };
 
@@ -247,6 +253,38 @@ struct Timed {  // brackets one kernel launch with events when profiling is on
   }
 };
 
+// ---- point-sharded mode: every partial sum over observations is summed over the shards before it is used ----
+// The data goes through the caller's exchange buffer: vec[0..n) (+ up to 4 scalars behind it), one call of the caller's
+// collective, and back.  op 0 = sum of doubles, op 1 = broadcast of bytes from the root shard.
+int shard_sum(caspar_ba* h, double* vec, size_t n, double* const* scalars, int ns, cudaStream_t s) {
+  if (!h->exchange) return 0;
+  if (n + (size_t)ns > h->xchg_count) return fail(h, CASPAR_BA_EINVAL, "exchange buffer too small");
+  if (n) CK(cudaMemcpyAsync(h->xchg, vec, n * sizeof(double), cudaMemcpyDeviceToDevice, s));
+  for (int i = 0; i < ns; ++i)
+    CK(cudaMemcpyAsync(h->xchg + n + i, scalars[i], sizeof(double), cudaMemcpyDeviceToDevice, s));
+  if (h->exchange(h->exchange_ctx, n + (size_t)ns, 0, (void*)s) != 0)
+    return fail(h, CASPAR_BA_ECUDA, "the shard exchange callback failed (sum)");
+  if (n) CK(cudaMemcpyAsync(vec, h->xchg, n * sizeof(double), cudaMemcpyDeviceToDevice, s));
+  for (int i = 0; i < ns; ++i)
+    CK(cudaMemcpyAsync(scalars[i], h->xchg + n + i, sizeof(double), cudaMemcpyDeviceToDevice, s));
+  ++h->exchanges;
+  return 0;
+}
+
+// The PCG scalars are sums folded with atomics (last-bit differences between shards); every decision taken from them
+// (alpha, beta, the power-of-two direction scale, done) must be the SAME on all shards: the root's copy is broadcast.
+int shard_broadcast_pcg(caspar_ba* h, cudaStream_t s) {
+  if (!h->exchange) return 0;
+  const size_t words = (sizeof(PcgScalars) + 7) / 8;
+  if (words > h->xchg_count) return fail(h, CASPAR_BA_EINVAL, "exchange buffer too small");
+  CK(cudaMemcpyAsync(h->xchg, h->v.pcg, sizeof(PcgScalars), cudaMemcpyDeviceToDevice, s));
+  if (h->exchange(h->exchange_ctx, sizeof(PcgScalars), 1, (void*)s) != 0)
+    return fail(h, CASPAR_BA_ECUDA, "the shard exchange callback failed (broadcast)");
+  CK(cudaMemcpyAsync(h->v.pcg, h->xchg, sizeof(PcgScalars), cudaMemcpyDeviceToDevice, s));
+  ++h->exchanges;
+  return 0;
+}
+
 int sync_step_scalars(caspar_ba* h, cudaStream_t s) {
   CK(cudaMemcpyAsync(h->h_step, h->v.step, sizeof(StepScalars), cudaMemcpyDeviceToHost, s));
   CK(cudaMemcpyAsync(h->h_pcg, h->v.pcg, sizeof(PcgScalars), cudaMemcpyDeviceToHost, s));
@@ -266,6 +304,11 @@ int do_linearize(caspar_ba* h, cudaStream_t s) {
   }
   CK(launch_linearize_cost(v, &v.step->cost, s));
   CK(launch_assemble_cameras(v, s));
+  {  // shards: U_j, g_c,j and the cost are sums over every shard's observations
+    double* sc[1] = {&v.step->cost};
+    int rc = shard_sum(h, v.Ug, (size_t)kUg * (size_t)v.nc, sc, 1, s);
+    if (rc) return rc;
+  }
   account(h);
   h->linearized = true;
   h->prepared = false;
@@ -275,7 +318,14 @@ int do_linearize(caspar_ba* h, cudaStream_t s) {
 
 int do_prepare(caspar_ba* h, double lambda, int preconditioner, cudaStream_t s) {
   if (h->prepared && h->prepared_lambda == lambda && h->prepared_preconditioner == preconditioner) return 0;
-  CK(launch_prepare_blocks(h->v, lambda, preconditioner, s));
+  if (h->exchange && preconditioner == 1) {  // the Schur-diagonal sums run over every shard's observations
+    CK(launch_prepare_blocks(h->v, lambda, preconditioner, s, 1));
+    int rc = shard_sum(h, h->v.Sdiag, 45 * (size_t)h->v.nc, nullptr, 0, s);
+    if (rc) return rc;
+    CK(launch_prepare_blocks(h->v, lambda, preconditioner, s, 2));
+  } else {
+    CK(launch_prepare_blocks(h->v, lambda, preconditioner, s));
+  }
   account(h);
   h->prepared = true;
   h->prepared_lambda = lambda;
@@ -308,13 +358,24 @@ static void build_chunk_graph(caspar_ba* h) {
 int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream_t s) {
   View& v = h->v;
   h->prepared = false;  // the right-hand side b is rebuilt by prepare (it starts from -g_c)
-  CK(cudaMemsetAsync(&v.step->jd2, 0, 2 * sizeof(double) + 2 * sizeof(int), s));  // jd2, dg, bad_block
+  CK(cudaMemsetAsync(&v.step->jd2, 0, 3 * sizeof(double), s));  // jd2, dg, bad_block
   int rc = do_prepare(h, lambda, h->preconditioner, s);
   if (rc) return rc;
   CK(cudaMemsetAsync(v.pcg, 0, sizeof(PcgScalars), s));
   CK(launch_schur_rhs(v, s));
+  rc = shard_sum(h, v.b, 9 * (size_t)v.nc, nullptr, 0, s);  // b = -g_c (root only) + sum over shards of W V'^-1 g_p
+  if (rc) return rc;
   const double tol2 = rel_tol * rel_tol;
-  CK(launch_pcg_init(v, tol2, s));
+  if (h->exchange) {  // |b|^2 fixes the direction scale of pcg_init: broadcast between the two kernels and after
+    CK(launch_pcg_init(v, tol2, s, 1));
+    rc = shard_broadcast_pcg(h, s);
+    if (rc) return rc;
+    CK(launch_pcg_init(v, tol2, s, 2));
+    rc = shard_broadcast_pcg(h, s);
+    if (rc) return rc;
+  } else {
+    CK(launch_pcg_init(v, tol2, s));
+  }
   const int chunk = kPcgChunk;
   // whole chunks go out as one graph launch (not while per-launch profiling events are wanted)
   if (!h->graph_tried[h->set_parity] && v.nc > 0 && v.num_tiles > 0) {  // the kernel arguments hold the set's pointers
@@ -322,7 +383,7 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
     build_chunk_graph(h);
   }
   cudaGraphExec_t chunk_graph = h->chunk_graph[h->set_parity];
-  const bool use_graph = chunk_graph != nullptr && !h->profiling;
+  const bool use_graph = chunk_graph != nullptr && !h->profiling && !h->exchange;
   int polled = 0;  // chunks whose flag copy has been enqueued
   bool stop = false;
   for (int it = 0; it < max_iter && !stop; ++it) {
@@ -335,8 +396,22 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
         Timed t(h, &h->ev_mv, s);
         CK(launch_schur_matvec(v, s));
       }
-      CK(launch_pcg_update(v, s));
+      if (h->exchange) {  // q and p.q are sums over the shards; then the root's scalars after each update kernel
+        double* sc[1] = {&v.pcg->pq};
+        rc = shard_sum(h, v.q, 9 * (size_t)v.nc, sc, 1, s);
+        if (rc) return rc;
+        CK(launch_pcg_update(v, s, 1));
+        rc = shard_broadcast_pcg(h, s);
+        if (rc) return rc;
+        CK(launch_pcg_update(v, s, 2));
+        rc = shard_broadcast_pcg(h, s);
+        if (rc) return rc;
+      } else {
+        CK(launch_pcg_update(v, s));
+      }
     }
+    // (shards: the flag copied here is the broadcast one and the copy sits at the same place of every shard's stream,
+    // so all shards read the same value and stop after the same chunk: the collectives stay matched)
     if (rel_tol > 0.0 && (it + 1) % chunk == 0 && it + 1 < max_iter) {
       const int slot = polled & 1;
       if (polled >= 2) {  // wait for the copy enqueued two chunks ago (slot reuse) and look at it
@@ -361,7 +436,8 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
 int do_pcgnr(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream_t s) {
   View& v = h->v;
   h->prepared = false;  // b is rebuilt by prepare (it starts from -g_c)
-  CK(cudaMemsetAsync(&v.step->jd2, 0, 2 * sizeof(double) + 2 * sizeof(int), s));  // jd2, dg, bad_block
+  if (h->exchange) return fail(h, CASPAR_BA_ESTATE, "the full-system solve (N1) is not available on a sharded handle");
+  CK(cudaMemsetAsync(&v.step->jd2, 0, 3 * sizeof(double), s));  // jd2, dg, bad_block
   int rc = do_prepare(h, lambda, 0, s);  // one block per node: U'_j and V'_k
   if (rc) return rc;
   CK(cudaMemsetAsync(v.pcg, 0, sizeof(PcgScalars), s));
@@ -479,6 +555,7 @@ static int create_impl(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba
   v.robust_inv_c2 = pb->robust_loss ? 1.0 / ((double)pb->robust_scale * (double)pb->robust_scale) : 0.0;
   v.damping_mode = pb->damping_mode;
   v.camera_model = pb->camera_model;
+  v.shard_root = 1;
   v.depth_eps = pb->depth_epsilon;
   v.cameras = pb->cameras;
   v.points = pb->points;
@@ -611,7 +688,9 @@ int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
   CK(launch_camera_prepass(v, v.cameras, v.cam_table_trial, s));
   CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
   account(h);
-  int rc = sync_step_scalars(h, s);
+  int rc = shard_sum(h, &v.step->trial_cost, 1, nullptr, 0, s);
+  if (rc) return rc;
+  rc = sync_step_scalars(h, s);
   if (rc) return rc;
   *cost_out = 0.5 * h->h_step->trial_cost;
   return std::isfinite(*cost_out) ? CASPAR_BA_OK : fail(h, CASPAR_BA_ENUMERIC, "non-finite cost");
@@ -624,6 +703,8 @@ int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max
   cudaStream_t s = (cudaStream_t)cuda_stream;
   DeviceGuard on_device(h->device);
   int rc = do_pcg(h, (double)lambda, (double)rel_tol, max_iter, s);
+  if (rc) return rc;
+  rc = shard_sum(h, &h->v.step->jd2, 3, nullptr, 0, s);  // shards: jd2, dg, bad_block
   if (rc) return rc;
   rc = sync_step_scalars(h, s);
   if (rc) return rc;
@@ -675,7 +756,7 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   // other set of arrays; if the step is accepted that IS the next iteration's linearization ("the
   // initial score and the Jacobian are calculated simultaneously, while subsequent runs use the score values from the
   // previous iteration").  (A forced rejection, accept_mode 2, speculates too: the tests use it for rejected steps.)
-  const bool speculate = h->fusion != 0 && h->arena2 != nullptr;
+  const bool speculate = h->fusion != 0 && h->arena2 != nullptr && !h->exchange;  // (not on a sharded handle)
   if (speculate) {
     View w = v;
     for (int i = 0; i < 6; ++i) w.J[i] = h->alt.J[i];
@@ -688,6 +769,9 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   } else {
     CK(launch_cost(v, v.pts_trial, v.cam_table_trial, &v.step->trial_cost, s));
   }
+  // shards: the trial cost, |J delta|^2, delta.g and the bad-block count are sums over the shards (contiguous scalars)
+  rc = shard_sum(h, &v.step->trial_cost, 4, nullptr, 0, s);
+  if (rc) return rc;
   account(h);
   rc = sync_step_scalars(h, s);  // the one host synchronisation of the step
   if (rc) return rc;
@@ -746,6 +830,31 @@ int caspar_ba_lm_step(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_i
   } else if (speculate) {
     ++h->speculative_misses;
   }
+  return CASPAR_BA_OK;
+}
+
+int caspar_ba_set_shard(caspar_ba_t* h, caspar_ba_exchange_fn fn, void* ctx, double* exchange_buffer_dev,
+                        size_t exchange_count, int32_t is_root) {
+  if (!h) return CASPAR_BA_EINVAL;
+  if (!fn) {  // back to a single-GPU problem
+    h->exchange = nullptr;
+    h->exchange_ctx = nullptr;
+    h->xchg = nullptr;
+    h->xchg_count = 0;
+    h->v.shard_root = 1;
+  } else {
+    const size_t need = (size_t)kUg * (size_t)h->v.nc + 8;
+    if (!exchange_buffer_dev || exchange_count < need || exchange_count < (sizeof(PcgScalars) + 7) / 8)
+      return fail(h, CASPAR_BA_EINVAL, "exchange buffer: need at least 54 * num_cameras + 8 doubles (" + std::to_string(need) + ")");
+    h->exchange = fn;
+    h->exchange_ctx = ctx;
+    h->xchg = exchange_buffer_dev;
+    h->xchg_count = exchange_count;
+    h->v.shard_root = is_root ? 1 : 0;
+  }
+  h->linearized = false;
+  h->prepared = false;
+  h->have_delta = false;
   return CASPAR_BA_OK;
 }
 
@@ -865,7 +974,14 @@ int caspar_ba_schur_matvec(caspar_ba_t* h, float lambda, const double* p_dev, do
   CK(cudaMemsetAsync(h->v.pcg, 0, sizeof(PcgScalars), s));
   {
     Timed t(h, &h->ev_mv, s);  // brackets load + pass + finish; the pass dominates
-    CK(launch_matvec_standalone(h->v, p_dev, q_dev, s));
+    if (h->exchange) {
+      CK(launch_matvec_standalone(h->v, p_dev, q_dev, s, 1));
+      rc = shard_sum(h, h->v.q, 9 * (size_t)h->v.nc, nullptr, 0, s);
+      if (rc) return rc;
+      CK(launch_matvec_standalone(h->v, p_dev, q_dev, s, 2));
+    } else {
+      CK(launch_matvec_standalone(h->v, p_dev, q_dev, s));
+    }
   }
   account(h);
   h->have_delta = false;  // x / p buffers were reused
@@ -907,6 +1023,7 @@ int caspar_ba_get_stats(caspar_ba_t* h, caspar_ba_stats* out) {
   out->speculative_hits = h->speculative_hits;
   out->speculative_misses = h->speculative_misses;
   out->arena2_bytes = (int64_t)h->arena2_bytes;
+  out->shard_exchanges = h->exchanges;
   return CASPAR_BA_OK;
 }
 

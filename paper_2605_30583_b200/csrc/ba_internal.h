@@ -57,8 +57,7 @@ struct StepScalars {
   double trial_cost;  // same at the trial point
   double jd2;         // |J delta|^2
   double dg;          // delta.g
-  int bad_block;      // a 9x9 / 3x3 block was not positive definite
-  int pad;
+  double bad_block;   // > 0: a 9x9 / 3x3 block was not positive definite (a double so that shards can sum it)
 };
 
 // Everything the kernels need, passed by value.
@@ -71,6 +70,8 @@ struct View {
   float robust_c2;
   double robust_inv_c2;  // 1 / c^2
   int damping_mode;
+  int shard_root;    // 1 unless this handle is a non-root shard of a point-sharded problem (caspar_ba_set_shard): only
+                     // the root adds the replicated camera terms (-g_c in b, delta_c.g_c) that the shards then sum
   int camera_model;  // 0: angle-axis, additive; 1: Pose3 tangent-space rotation (right perturbation) + retraction
   float depth_eps;   // d_safe = d + eps sign_no_zero(d); 0 = no guard
   // caller's arrays (borrowed)
@@ -187,16 +188,19 @@ cudaError_t launch_linearize_at(const View& v, const float4* pts, const float* t
 cudaError_t launch_linearize_cost(const View& v, double* cost_out, cudaStream_t s);  // folds launch_linearize's partials
 cudaError_t launch_cost(const View& v, const float4* pts, const float* table, double* cost_out, cudaStream_t s);
 cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s);
-cudaError_t launch_prepare_blocks(const View& v, double lambda, int preconditioner, cudaStream_t s);
+// `stage`: 0 = everything; 1 = point blocks (+ the Schur-diagonal sums for preconditioner 1) only; 2 = camera blocks only
+// (a sharded handle sums Sdiag over the shards between 1 and 2)
+cudaError_t launch_prepare_blocks(const View& v, double lambda, int preconditioner, cudaStream_t s, int stage = 0);
 cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);
-cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s);
+// `stage` (sharded handles): 0 = both kernels, 1 = the first only, 2 = the second only
+cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s, int stage = 0);
 cudaError_t launch_schur_matvec(const View& v, cudaStream_t s);
 cudaError_t configure_kernels(const View& v);  // once per handle: dynamic shared memory opt-in
 bool pipelined_matvec_possible(const View& v);   // shape / shared-memory check, at create
 bool pipelined_linearize_possible(const View& v);
 bool pipelined_matvec_available(const View& v);  // = v.pipeline
 int pipeline_stages(const View& v);
-cudaError_t launch_pcg_update(const View& v, cudaStream_t s);  // two kernels
+cudaError_t launch_pcg_update(const View& v, cudaStream_t s, int stage = 0);  // two kernels
 cudaError_t launch_backsub(const View& v, cudaStream_t s);
 cudaError_t launch_full_matvec(const View& v, cudaStream_t s);
 cudaError_t launch_pcgnr_init(const View& v, double lambda, double tol2, cudaStream_t s);
@@ -205,6 +209,7 @@ cudaError_t launch_pcgnr_finish(const View& v, cudaStream_t s);
 cudaError_t launch_trial_update(const View& v, cudaStream_t s);
 cudaError_t launch_commit(const View& v, cudaStream_t s);
 cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s);
-cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s);
+// `stage` (sharded handles): 0 = all, 1 = load + pass (leaves the shard's partial in v.q), 2 = finish (adds lambda D p)
+cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s, int stage = 0);
 
 }  // namespace cba

@@ -878,7 +878,7 @@ __global__ void prepare_cameras_kernel(View v, double lambda, int schur_diagonal
     const double d = v.damping_mode == 1 ? 1.0 : fmax(A[10 * a], (double)kDMin);
     ld[a] = lambda * d;
     v.lamD[9ll * j + a] = ld[a];
-    v.b[9ll * j + a] = -ug[45 + a];
+    v.b[9ll * j + a] = v.shard_root ? -ug[45 + a] : 0.0;  // the shards' right-hand sides are summed: -g_c enters once
   }
   if (schur_diagonal) {  // S_jj = lambda D_j + sum J_c^T (I - B) J_c
     const double* sd = v.Sdiag + 45ll * j;
@@ -910,7 +910,7 @@ __global__ void prepare_cameras_kernel(View v, double lambda, int schur_diagonal
     }
   double* Mi = v.Minv + 81ll * j;
   if (!ok) {
-    v.step->bad_block = 1;
+    v.step->bad_block = 1.0;
     for (int i = 0; i < 81; ++i) Mi[i] = (i % 10 == 0) ? 1.0 : 0.0;
     return;
   }
@@ -944,7 +944,7 @@ __global__ void prepare_points_kernel(View v, double lambda) {
   const double l00 = xx, l10 = xy / l00, l20 = xz / l00;
   const double d1 = yy - l10 * xy, m21 = yz - l10 * xz, d2 = zz - l20 * xz - (m21 / d1) * m21;
   if (!(l00 > 0.0) || !(d1 > 0.0) || !(d2 > 0.0)) {
-    v.step->bad_block = 1;
+    v.step->bad_block = 1.0;
     v.Vinv[2ll * k] = make_float4(0.f, 0.f, 0.f, 0.f);
     v.Vinv[2ll * k + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int i = 0; i < 6; ++i) v.Vinv64[6ll * k + i] = 0.0;
@@ -1851,7 +1851,7 @@ __global__ void __launch_bounds__(kPcgThreads) delta_c_kernel(View v) {
   if (j < v.nc) {
     const double xi = v.x[i];
     v.p32[(long long)kCamPad * j + a] = (float)xi;
-    d = xi * v.Ug[(long long)kUg * j + 45 + a];
+    d = v.shard_root ? xi * v.Ug[(long long)kUg * j + 45 + a] : 0.0;  // delta_c.g_c enters the shards' sum once
   }
   const double s = block_sum(d, red);
   if (threadIdx.x == 0) atomicAdd(&v.step->dg, s);
@@ -2095,8 +2095,15 @@ cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s) {
 
 // preconditioner: 0 = blockdiag(U'_j) (C9), 1 = the diagonal blocks of S (N4; needs V'^-1 first, and one more
 // camera-ordered pass over the Jacobians)
-cudaError_t launch_prepare_blocks(const View& v, double lambda, int preconditioner, cudaStream_t s) {
+cudaError_t launch_prepare_blocks(const View& v, double lambda, int preconditioner, cudaStream_t s, int stage) {
   cudaError_t e = cudaSuccess;
+  if (stage == 2) {
+    if (v.nc > 0) {
+      prepare_cameras_kernel<<<grid_for(v.nc, 64), 64, 0, s>>>(v, lambda, preconditioner);
+      e = CBA_LAUNCHED();
+    }
+    return e;
+  }
   if (v.np_obs > 0) {
     prepare_points_kernel<<<grid_for(v.np_obs, 256), 256, 0, s>>>(v, lambda);
     e = CBA_LAUNCHED();
@@ -2111,7 +2118,7 @@ cudaError_t launch_prepare_blocks(const View& v, double lambda, int precondition
       e = CBA_LAUNCHED();
     }
   }
-  if (e == cudaSuccess && v.nc > 0) {
+  if (e == cudaSuccess && v.nc > 0 && stage == 0) {
     prepare_cameras_kernel<<<grid_for(v.nc, 64), 64, 0, s>>>(v, lambda, preconditioner);
     e = CBA_LAUNCHED();
   }
@@ -2220,21 +2227,27 @@ static cudaError_t launch_pipelined_or_pass(const View& v, cudaStream_t s) {
 
 cudaError_t launch_schur_matvec(const View& v, cudaStream_t s) { return launch_pipelined_or_pass<MATVEC>(v, s); }
 
-cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s) {
+cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s, int stage) {
   if (v.nc == 0) return cudaSuccess;
-  pcg_norm_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
-  cudaError_t e = CBA_LAUNCHED();
-  if (e != cudaSuccess) return e;
+  cudaError_t e = cudaSuccess;
+  if (stage != 2) {
+    pcg_norm_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
+    e = CBA_LAUNCHED();
+  }
+  if (e != cudaSuccess || stage == 1) return e;
   pcg_init_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v, tol2);
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_pcg_update(const View& v, cudaStream_t s) {
+cudaError_t launch_pcg_update(const View& v, cudaStream_t s, int stage) {
   if (v.nc == 0) return cudaSuccess;
   const unsigned g = grid_for(9ll * v.nc, kPcgThreads);
-  pcg_update_xr_kernel<<<g, kPcgThreads, 0, s>>>(v);
-  cudaError_t e = CBA_LAUNCHED();
-  if (e != cudaSuccess) return e;
+  cudaError_t e = cudaSuccess;
+  if (stage != 2) {
+    pcg_update_xr_kernel<<<g, kPcgThreads, 0, s>>>(v);
+    e = CBA_LAUNCHED();
+  }
+  if (e != cudaSuccess || stage == 1) return e;
   pcg_update_p_kernel<<<g, kPcgThreads, 0, s>>>(v);
   return CBA_LAUNCHED();
 }
@@ -2349,14 +2362,17 @@ cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s) 
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s) {
+cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s, int stage) {
   if (v.nc == 0) return cudaSuccess;
   const unsigned g = grid_for(9ll * v.nc, 256);
-  matvec_load_kernel<<<g, 256, 0, s>>>(v, p_in);
-  cudaError_t e = CBA_LAUNCHED();
-  if (e != cudaSuccess) return e;
-  e = launch_schur_matvec(v, s);
-  if (e != cudaSuccess) return e;
+  cudaError_t e = cudaSuccess;
+  if (stage != 2) {
+    matvec_load_kernel<<<g, 256, 0, s>>>(v, p_in);
+    e = CBA_LAUNCHED();
+    if (e != cudaSuccess) return e;
+    e = launch_schur_matvec(v, s);
+  }
+  if (e != cudaSuccess || stage == 1) return e;
   matvec_finish_kernel<<<g, 256, 0, s>>>(v, q_out);
   return CBA_LAUNCHED();
 }
