@@ -10,8 +10,11 @@ the scene the north_star's roofline target is quoted on.  The timed K steps are 
 the adaptive LM schedule from the perturbed start (lambda0 = 1e-2); the W warm-up steps run first and the
 parameters are then reset.  One JSON line is printed by rank 0.
 
-N > 1 (torchrun): the path is single-GPU (north_star); ranks run independent replicas of the config with
-different seeds and no data-path collective ("scaling": "weak"); time = max over ranks.
+N > 1 (torchrun): the path is single-GPU (north_star); by default ranks run independent replicas of the config with
+different seeds and no data-path collective ("scaling": "weak"); time = max over ranks.  `--parallelism sharded` runs
+ONE problem instead, its points split over the ranks (caspar_ba_set_shard with NCCL all-reduce /
+broadcast through torch.distributed): "scaling": "strong".  That mode has only ever run on one GPU (world size 1 and
+two emulated ranks in tests/test_gpu_sharding.py): no multi-GPU box was available to this build.
 """
 from __future__ import annotations
 
@@ -245,12 +248,27 @@ def run_ours(args):
     kw = {}
     if args.shrink:                                   # debugging only; the bench line says so
         kw = SAMPLES[args.workload]
-    scene = make_scene(args.workload, seed=replica_seed(cfg["seed"], rank), **kw)
+    sharded = args.parallelism == "sharded"
+    scene = make_scene(args.workload, seed=cfg["seed"] if sharded else replica_seed(cfg["seed"], rank), **kw)
     n_obs = scene.num_observations
+    full_scene = scene
+    if sharded:   # every rank builds the same scene and keeps its own range of points (whole tracks)
+        import dataclasses
+        from paper_2605_30583_b200 import sharding
+        sh = sharding.make_shard(scene.num_points, scene.camera_index, scene.point_index, world, rank)
+        pts_l, obs_l = sharding.shard_arrays(sh, scene.points, scene.observations)
+        scene = dataclasses.replace(scene, points=np.ascontiguousarray(pts_l), observations=np.ascontiguousarray(obs_l),
+                                    camera_index=sh.camera_index, point_index=sh.point_index)
     cams0 = torch.from_numpy(scene.cameras).to(dev)
     pts0 = torch.from_numpy(scene.points).to(dev)
     gpu = pkg.CasparBA(cams0.clone(), pts0.clone(), scene.observations, scene.camera_index, scene.point_index,
                        scene.robust_loss, scene.robust_scale, 0, device=dev)
+    if sharded:
+        if world == 1 and not dist.is_initialized():
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29655")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+        gpu.set_shard(sharding.torch_exchange(), is_root=(rank == 0))
     tol, cap = cfg["pcg_rel_tol"], cfg["pcg_max_iter"]
 
     cam_h = torch.empty((scene.num_cameras, 9), dtype=torch.float32).pin_memory()
@@ -330,7 +348,7 @@ def run_ours(args):
     param_bytes = 4 * (9 * scene.num_cameras + 3 * scene.num_points)
 
     if rank != 0:
-        if world > 1:
+        if dist.is_initialized():
             dist.destroy_process_group()
         return
 
@@ -340,8 +358,9 @@ def run_ours(args):
     # algorithmic bytes:
     #   matvec   : J_c 72 + J_p 24 + camera id 4 per observation, V'^-1 24 per observed point
     #   linearize: pixel 8 + camera id 4 + r 8 + J_c 72 + J_p 24 per observation, X 12 + V,g_p 36 per point
-    mv_bytes = 100.0 * n_obs + 24.0 * observed_points
-    lin_bytes = 116.0 * n_obs + 48.0 * observed_points
+    n_local = scene.num_observations          # = n_obs unless the problem is sharded (then: this rank's share)
+    mv_bytes = 100.0 * n_local + 24.0 * observed_points
+    lin_bytes = 116.0 * n_local + 48.0 * observed_points
     # launches enqueued after the device-side convergence flag was set return at once (a few us each):
     # their time is kept in the total, but the average is over the matvecs that ran
     mv_ms = st.matvec_ms_total / max(1, matvecs_prof)
@@ -349,18 +368,23 @@ def run_ours(args):
     mv_gbs = mv_bytes / (mv_ms * 1e-3) / 1e9 if mv_ms > 0 else 0.0
     lin_gbs = lin_bytes / (lin_ms * 1e-3) / 1e9 if lin_ms > 0 else 0.0
 
-    value = whole_job_rate(world, args.steps, ms_max)
+    # replicas: every rank did K steps of its own problem; sharded: the ranks did K steps of ONE problem together
+    value = args.steps / (ms_max * 1e-3) if sharded else whole_job_rate(world, args.steps, ms_max)
     line = {
         "metric": "lm_iterations_per_s", "value": value, "unit": "LM iterations/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[3] '{args.workload}' (seed {cfg['seed']})" + (" SHRUNK (debug)" if args.shrink else ""),
-                   "cameras": scene.num_cameras, "points": scene.num_points, "observations": n_obs,
+        "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{['tiny', 'small', 'mid', 'large', 'skewed'].index(args.workload)}] '{args.workload}' (seed {cfg['seed']})" + (" SHRUNK (debug)" if args.shrink else ""),
+                   "cameras": full_scene.num_cameras, "points": full_scene.num_points, "observations": n_obs,
                    "pcg_max_iter": cap, "pcg_rel_tol": tol, "lambda0": LAMBDA0, "tile_slots": int(st.tile_slots),
                    "l2": "inputs larger than L2 (stored Jacobians %.2f GB per pass)" % (96.0 * n_obs / 1e9),
-                   "replicas": world, "parallelism": "independent replicas, no collective"},
-        "schur_matvecs_per_s": whole_job_rate(world, matvecs, ms_max), "matvecs_in_timed_region": matvecs,
-        "linearizations_per_s": n_obs / (lin_ms * 1e-3) if lin_ms > 0 else None,
+                   "replicas": 1 if sharded else world,
+                   "parallelism": (f"points sharded over {world} rank(s): all-reduce of U/g_c, b, every q (9 Nc doubles) and "
+                                   f"the step scalars, broadcast of the PCG scalars; {int(st.shard_exchanges)} collectives in the profiled pass")
+                   if sharded else "independent replicas, no collective"},
+        "schur_matvecs_per_s": (matvecs / (ms_max * 1e-3)) if sharded else whole_job_rate(world, matvecs, ms_max),
+        "matvecs_in_timed_region": matvecs,
+        "linearizations_per_s": world * n_local / (lin_ms * 1e-3) if lin_ms > 0 else None,
         "lm_costs": [s.cost_after for s in steps], "lm_accepted": [bool(s.accepted) for s in steps],
         "pcg_iterations": [s.pcg_iterations for s in steps],
         "roofline": {"kernel": "schur_matvec_pipelined_kernel<T>" if st.matvec_pipelined else "schur_pass_kernel<T,MATVEC>", "bound": "hbm", "achieved": mv_gbs, "peak": peak,
@@ -373,7 +397,7 @@ def run_ours(args):
                                "unit": "GB/s", "frac": lin_gbs / peak, "traffic": ncu_traffic("linearize") if args.workload == "large" and not args.shrink else None,
                                "algorithmic_bytes_per_launch": lin_bytes, "avg_launch_ms": lin_ms,
                                "launches_timed": lin_count, "frac_of_nominal_8TBs": lin_gbs / 8000.0},
-        "e2e": {"value": world * args.steps / e2e_s, "unit": "LM iterations/s", "h2d_bytes_per_step": param_bytes,
+        "e2e": {"value": (1 if sharded else world) * args.steps / e2e_s, "unit": "LM iterations/s", "h2d_bytes_per_step": param_bytes,
                 "d2h_bytes_per_step": param_bytes + 88,
                 "what": "pinned host parameters -> caspar_ba_set_parameters_host, caspar_ba_lm_step, "
                         "caspar_ba_get_parameters_host + step_info, every step; wall clock"},
@@ -391,7 +415,7 @@ def run_ours(args):
         desc["single_thread"] = time_oracle_single_thread(args.workload)
         line["cpu_baseline"] = desc
     print(json.dumps(line), flush=True)
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 
@@ -403,6 +427,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="large", choices=list(SAMPLES))
     ap.add_argument("--shrink", action="store_true", help="debug: run the shrunken sample scene on the GPU")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
+                    help="N > 1: independent replicas (default, weak scaling) or ONE problem with its points sharded "
+                         "over the ranks (strong scaling; caspar_ba_set_shard over NCCL)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="profiling runs: skip the host-buffer end-to-end leg")
     args = ap.parse_args()
