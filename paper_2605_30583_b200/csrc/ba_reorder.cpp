@@ -113,6 +113,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
   {
     std::vector<unsigned long long> keys;
     std::vector<unsigned short> pid_of_r;
+    std::vector<unsigned char> taken;
 #pragma omp for schedule(dynamic, 64)
     for (int t = 0; t < num_tiles; ++t) {
       int base = out->pt_ptr[tile_pt[t]];
@@ -126,9 +127,31 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
         for (int r = out->pt_ptr[a] - base; r < out->pt_ptr[a + 1] - base; ++r) pid_of_r[r] = (unsigned short)(a - tile_pt[t]);
       long long s0 = (long long)t * T;
       int runs = 0, prev = -1;
+      // Bank-aware ranks.  A slot's rank must lie in its point's range [pt_ptr[k], pt_ptr[k + 1]) - base, but WHICH
+      // position of the range it takes is free.  The kernels scatter per-observation products to shared-memory rows
+      // indexed by rank (Schur matvec: 8-byte rows, 16 lanes per wavefront; linearize: 16-byte rows, 8 lanes per
+      // wavefront), and with ranks in point-major input order those stores ran at 2.9x their ideal wavefronts
+      // (profiles/r02_ncu_schur_matvec.md).  Greedy: walking the slots in order, a slot takes the free position of
+      // its point whose bank (rank mod 16, rank mod 8) is unused so far in its half-warp / quarter-warp.
+      taken.assign(cnt, 0);
+      unsigned half_used = 0, quarter_used = 0;
       for (int s = 0; s < cnt; ++s) {
-        int r = (int)(keys[s] & 0xFFFFu), c = (int)(keys[s] >> 16);
-        out->obs_of_slot[s0 + s] = obs_by_pt[base + r];
+        const int r0 = (int)(keys[s] & 0xFFFFu), c = (int)(keys[s] >> 16);
+        const int a = tile_pt[t] + pid_of_r[r0];
+        const int lo = out->pt_ptr[a] - base, hi = out->pt_ptr[a + 1] - base;
+        if ((s & 15) == 0) half_used = 0;
+        if ((s & 7) == 0) quarter_used = 0;
+        int best = -1, best_cost = 4;
+        for (int r = lo; r < hi && best_cost > 0; ++r) {
+          if (taken[r]) continue;
+          const int cost = 2 * (int)((half_used >> (r & 15)) & 1u) + (int)((quarter_used >> (r & 7)) & 1u);
+          if (cost < best_cost) { best_cost = cost; best = r; }
+        }
+        const int r = best;
+        taken[r] = 1;
+        half_used |= 1u << (r & 15);
+        quarter_used |= 1u << (r & 7);
+        out->obs_of_slot[s0 + s] = obs_by_pt[base + r0];
         out->cam[s0 + s] = c;
         out->rank[s0 + s] = (unsigned short)r;
         if (T <= 256) out->rankpid[s0 + s] = (unsigned short)(r | (pid_of_r[r] << 8));
