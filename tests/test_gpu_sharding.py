@@ -148,7 +148,8 @@ def test_sharded_lm_steps_match_and_the_shards_stay_replicas(scene_cache, precon
     ref.close()
     for r in out:
         for x, y in zip(r["steps"], want):
-            assert x.accepted == y.accepted and abs(x.pcg_iterations - y.pcg_iterations) <= 1
+            # (stopping on a tolerance: the residual hovers around it for a few iterations, C9)
+            assert x.accepted == y.accepted and abs(x.pcg_iterations - y.pcg_iterations) <= max(3, 0.1 * y.pcg_iterations)
             assert x.cost_before == pytest.approx(y.cost_before, rel=1e-6) and x.cost_after == pytest.approx(y.cost_after, rel=1e-6)
             assert x.rho == pytest.approx(y.rho, rel=1e-3)
         assert np.abs(r["cams"] - cams).max() <= 1e-4 * np.abs(cams).max()
