@@ -167,19 +167,18 @@ int caspar_ba_set_fusion(caspar_ba_t* h, int32_t mode);
  * POINT-SHARDED problem: the handle is ONE SHARD.  It was created with ALL cameras (replicated on every shard, the
  * same values) and a SUBSET of the points with all their observations (point ids local to the shard).  Every partial
  * sum over observations is then summed over the shards before it is used, through the caller's collective:
- *   fn(ctx, count, op, cuda_stream)  op 0: sum the first `count` DOUBLES of the exchange buffer over all shards, in
- *                                          place, result on every shard (an all-reduce);
- *                                    op 1: replace the first `count` BYTES of the buffer by the ROOT shard's
- *                                          (a broadcast);  both enqueued on `cuda_stream`; return 0 on success.
+ *   fn(ctx, count, cuda_stream)  sum the first `count` DOUBLES of the exchange buffer over all shards, in place, result
+ *                                on every shard (an all-reduce), enqueued on `cuda_stream`; return 0 on success.
  * exchange_buffer_dev: DEVICE, caller-owned, >= 54 * num_cameras + 8 doubles, borrowed until the next
  * caspar_ba_set_shard / destroy.  is_root: exactly one shard passes 1 (it contributes the replicated camera terms).
- * Exchanges per call: linearize 1 (U, g_c, cost); pcg_solve 1 (+1 with the Schur-Jacobi preconditioner) + 3 for the
- * right-hand side and the start + 3 per iteration (q and p.q summed; the root's PCG scalars broadcast after each of
- * the two update kernels so that alpha, beta, the direction scale and the stop decision are bit-identical on every
- * shard) + 1; lm_step adds 1 (trial cost, |J delta|^2, delta.g).  All shards must make the same calls in the same
- * order.  The CUDA-graph PCG chunks, caspar_ba_set_fusion and caspar_ba_pcgnr_solve are not used on a sharded handle.
+ * Exchanges per call: linearize 1 (U, g_c, cost); pcg_solve 1 for the right-hand side (+1 with the Schur-Jacobi
+ * preconditioner) + ONE per iteration (q and p.q) + 1 (step scalars); lm_step 1 more (trial cost, |J delta|^2,
+ * delta.g).  The PCG vector kernels run redundantly on every shard; their scalar sums are folded in a fixed order, so
+ * alpha, beta, the direction scale and the stop decision -- hence x, r, p and the cameras -- are bit-identical on all
+ * shards without any broadcast.  All shards must make the same calls in the same order.  The CUDA-graph PCG chunks,
+ * caspar_ba_set_fusion and caspar_ba_pcgnr_solve are not used on a sharded handle.
  * fn = NULL returns the handle to a single-GPU problem.  Errors: EINVAL (buffer too small). */
-typedef int (*caspar_ba_exchange_fn)(void* ctx, size_t count, int32_t op, void* cuda_stream);
+typedef int (*caspar_ba_exchange_fn)(void* ctx, size_t count, void* cuda_stream);
 int caspar_ba_set_shard(caspar_ba_t* h, caspar_ba_exchange_fn fn, void* ctx, double* exchange_buffer_dev,
                         size_t exchange_count, int32_t is_root);
 

@@ -60,8 +60,8 @@ class Stats(C.Structure):
                 ("shard_exchanges", C.c_int64)]
 
 
-# int fn(void* ctx, size_t count, int32_t op, void* cuda_stream)
-EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_size_t, C.c_int32, C.c_void_p)
+# int fn(void* ctx, size_t count, void* cuda_stream)
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_size_t, C.c_void_p)
 
 
 class LayoutInfo(C.Structure):
@@ -324,9 +324,9 @@ class CasparBA:
 
     def set_shard(self, exchange, is_root: bool):
         """Make this handle ONE SHARD of a point-sharded problem (include/caspar_ba.h: caspar_ba_set_shard).
-        `exchange(buffer, count, op)` is called with the handle's exchange buffer (a float64 CUDA tensor), on the
-        current stream: op 0 sums buffer[:count] over the shards in place, op 1 replaces the first `count` BYTES by the
-        root shard's.  `exchange=None` returns to a single-GPU problem.  See `sharding.torch_exchange`."""
+        `exchange(buffer, count)` is called with the handle's exchange buffer (a float64 CUDA tensor), on the current
+        stream: it sums buffer[:count] over the shards in place (an all-reduce).  `exchange=None` returns to a
+        single-GPU problem.  See `sharding.torch_exchange`."""
         if exchange is None:
             self._check(self._lib.caspar_ba_set_shard(self._h, EXCHANGE_FN(0), None, None, 0, 1), "set_shard")
             self._exchange_cb = self._xchg = None
@@ -334,9 +334,9 @@ class CasparBA:
         self._xchg = torch.zeros(54 * self.nc + 8, dtype=torch.float64, device=self.device)
         buf = self._xchg
 
-        def _cb(_ctx, count, op, _stream):
+        def _cb(_ctx, count, _stream):
             try:
-                exchange(buf, int(count), int(op))
+                exchange(buf, int(count))
                 return 0
             except Exception:  # never let an exception cross the C ABI
                 import traceback

@@ -190,6 +190,8 @@ size_t carve(caspar_ba* h, void* base, const Reordered& ro) {
   v.p = c.take<double>(9 * NC);
   v.q = c.take<double>(9 * NC);
   v.p32 = c.take<float>(kCamPad * NC);
+  v.pcg_part = c.take<double>(3 * (size_t)((9 * NC + 287) / 288 + 1));
+  v.pcg_ticket = c.take<unsigned>(1);
   v.pcg = c.take<PcgScalars>(1);
   v.step = c.take<StepScalars>(1);
   return (c.off + 255) & ~size_t(255);
@@ -255,32 +257,18 @@ struct Timed {  // brackets one kernel launch with events when profiling is on
 
 // ---- point-sharded mode: every partial sum over observations is summed over the shards before it is used ----
 // The data goes through the caller's exchange buffer: vec[0..n) (+ up to 4 scalars behind it), one call of the caller's
-// collective, and back.  op 0 = sum of doubles, op 1 = broadcast of bytes from the root shard.
+// collective (an all-reduce sum of doubles), and back.
 int shard_sum(caspar_ba* h, double* vec, size_t n, double* const* scalars, int ns, cudaStream_t s) {
   if (!h->exchange) return 0;
   if (n + (size_t)ns > h->xchg_count) return fail(h, CASPAR_BA_EINVAL, "exchange buffer too small");
   if (n) CK(cudaMemcpyAsync(h->xchg, vec, n * sizeof(double), cudaMemcpyDeviceToDevice, s));
   for (int i = 0; i < ns; ++i)
     CK(cudaMemcpyAsync(h->xchg + n + i, scalars[i], sizeof(double), cudaMemcpyDeviceToDevice, s));
-  if (h->exchange(h->exchange_ctx, n + (size_t)ns, 0, (void*)s) != 0)
-    return fail(h, CASPAR_BA_ECUDA, "the shard exchange callback failed (sum)");
+  if (h->exchange(h->exchange_ctx, n + (size_t)ns, (void*)s) != 0)
+    return fail(h, CASPAR_BA_ECUDA, "the shard exchange callback failed");
   if (n) CK(cudaMemcpyAsync(vec, h->xchg, n * sizeof(double), cudaMemcpyDeviceToDevice, s));
   for (int i = 0; i < ns; ++i)
     CK(cudaMemcpyAsync(scalars[i], h->xchg + n + i, sizeof(double), cudaMemcpyDeviceToDevice, s));
-  ++h->exchanges;
-  return 0;
-}
-
-// The PCG scalars are sums folded with atomics (last-bit differences between shards); every decision taken from them
-// (alpha, beta, the power-of-two direction scale, done) must be the SAME on all shards: the root's copy is broadcast.
-int shard_broadcast_pcg(caspar_ba* h, cudaStream_t s) {
-  if (!h->exchange) return 0;
-  const size_t words = (sizeof(PcgScalars) + 7) / 8;
-  if (words > h->xchg_count) return fail(h, CASPAR_BA_EINVAL, "exchange buffer too small");
-  CK(cudaMemcpyAsync(h->xchg, h->v.pcg, sizeof(PcgScalars), cudaMemcpyDeviceToDevice, s));
-  if (h->exchange(h->exchange_ctx, sizeof(PcgScalars), 1, (void*)s) != 0)
-    return fail(h, CASPAR_BA_ECUDA, "the shard exchange callback failed (broadcast)");
-  CK(cudaMemcpyAsync(h->v.pcg, h->xchg, sizeof(PcgScalars), cudaMemcpyDeviceToDevice, s));
   ++h->exchanges;
   return 0;
 }
@@ -366,16 +354,9 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
   rc = shard_sum(h, v.b, 9 * (size_t)v.nc, nullptr, 0, s);  // b = -g_c (root only) + sum over shards of W V'^-1 g_p
   if (rc) return rc;
   const double tol2 = rel_tol * rel_tol;
-  if (h->exchange) {  // |b|^2 fixes the direction scale of pcg_init: broadcast between the two kernels and after
-    CK(launch_pcg_init(v, tol2, s, 1));
-    rc = shard_broadcast_pcg(h, s);
-    if (rc) return rc;
-    CK(launch_pcg_init(v, tol2, s, 2));
-    rc = shard_broadcast_pcg(h, s);
-    if (rc) return rc;
-  } else {
-    CK(launch_pcg_init(v, tol2, s));
-  }
+  // (the scalar sums of the S7 kernels are deterministic -- fold_block_sums -- so every shard computes the same alpha,
+  // beta, direction scale and stop decision from the same summed b, q and p.q: no further exchange is needed)
+  CK(launch_pcg_init(v, tol2, s));
   const int chunk = kPcgChunk;
   // whole chunks go out as one graph launch (not while per-launch profiling events are wanted)
   if (!h->graph_tried[h->set_parity] && v.nc > 0 && v.num_tiles > 0) {  // the kernel arguments hold the set's pointers
@@ -396,22 +377,15 @@ int do_pcg(caspar_ba* h, double lambda, double rel_tol, int max_iter, cudaStream
         Timed t(h, &h->ev_mv, s);
         CK(launch_schur_matvec(v, s));
       }
-      if (h->exchange) {  // q and p.q are sums over the shards; then the root's scalars after each update kernel
+      if (h->exchange) {  // q and p.q are sums over the shards: the ONE exchange of a PCG iteration
         double* sc[1] = {&v.pcg->pq};
         rc = shard_sum(h, v.q, 9 * (size_t)v.nc, sc, 1, s);
         if (rc) return rc;
-        CK(launch_pcg_update(v, s, 1));
-        rc = shard_broadcast_pcg(h, s);
-        if (rc) return rc;
-        CK(launch_pcg_update(v, s, 2));
-        rc = shard_broadcast_pcg(h, s);
-        if (rc) return rc;
-      } else {
-        CK(launch_pcg_update(v, s));
       }
+      CK(launch_pcg_update(v, s));
     }
-    // (shards: the flag copied here is the broadcast one and the copy sits at the same place of every shard's stream,
-    // so all shards read the same value and stop after the same chunk: the collectives stay matched)
+    // (shards: every shard computes the same flag and the copy sits at the same place of every shard's stream, so all
+    // shards read the same value and stop after the same chunk: the collectives stay matched)
     if (rel_tol > 0.0 && (it + 1) % chunk == 0 && it + 1 < max_iter) {
       const int slot = polled & 1;
       if (polled >= 2) {  // wait for the copy enqueued two chunks ago (slot reuse) and look at it
@@ -842,15 +816,17 @@ int caspar_ba_set_shard(caspar_ba_t* h, caspar_ba_exchange_fn fn, void* ctx, dou
     h->xchg = nullptr;
     h->xchg_count = 0;
     h->v.shard_root = 1;
+    h->v.det_scalars = 0;
   } else {
     const size_t need = (size_t)kUg * (size_t)h->v.nc + 8;
-    if (!exchange_buffer_dev || exchange_count < need || exchange_count < (sizeof(PcgScalars) + 7) / 8)
+    if (!exchange_buffer_dev || exchange_count < need)
       return fail(h, CASPAR_BA_EINVAL, "exchange buffer: need at least 54 * num_cameras + 8 doubles (" + std::to_string(need) + ")");
     h->exchange = fn;
     h->exchange_ctx = ctx;
     h->xchg = exchange_buffer_dev;
     h->xchg_count = exchange_count;
     h->v.shard_root = is_root ? 1 : 0;
+    h->v.det_scalars = 1;
   }
   h->linearized = false;
   h->prepared = false;

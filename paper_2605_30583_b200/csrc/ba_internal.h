@@ -70,6 +70,7 @@ struct View {
   float robust_c2;
   double robust_inv_c2;  // 1 / c^2
   int damping_mode;
+  int det_scalars;   // 1: the S7 kernels fold their scalar sums in a fixed order (sharded handles), 0: one atomic per block
   int shard_root;    // 1 unless this handle is a non-root shard of a point-sharded problem (caspar_ba_set_shard): only
                      // the root adds the replicated camera terms (-g_c in b, delta_c.g_c) that the shards then sum
   int camera_model;  // 0: angle-axis, additive; 1: Pose3 tangent-space rotation (right perturbation) + retraction
@@ -147,6 +148,8 @@ struct View {
   int num_hot;
   PcgScalars* pcg;
   StepScalars* step;
+  double* pcg_part;         // [3][blocks of the S7 kernels] per-block partial sums, folded in block order by the last block
+  unsigned* pcg_ticket;     // blocks of the running S7 kernel that have stored their partials (back at 0 when it ends)
 };
 
 // Host-side result of the S0 reordering (ba_reorder.cpp).
@@ -192,15 +195,14 @@ cudaError_t launch_assemble_cameras(const View& v, cudaStream_t s);
 // (a sharded handle sums Sdiag over the shards between 1 and 2)
 cudaError_t launch_prepare_blocks(const View& v, double lambda, int preconditioner, cudaStream_t s, int stage = 0);
 cudaError_t launch_schur_rhs(const View& v, cudaStream_t s);
-// `stage` (sharded handles): 0 = both kernels, 1 = the first only, 2 = the second only
-cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s, int stage = 0);
+cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s);
 cudaError_t launch_schur_matvec(const View& v, cudaStream_t s);
 cudaError_t configure_kernels(const View& v);  // once per handle: dynamic shared memory opt-in
 bool pipelined_matvec_possible(const View& v);   // shape / shared-memory check, at create
 bool pipelined_linearize_possible(const View& v);
 bool pipelined_matvec_available(const View& v);  // = v.pipeline
 int pipeline_stages(const View& v);
-cudaError_t launch_pcg_update(const View& v, cudaStream_t s, int stage = 0);  // two kernels
+cudaError_t launch_pcg_update(const View& v, cudaStream_t s);  // two kernels
 cudaError_t launch_backsub(const View& v, cudaStream_t s);
 cudaError_t launch_full_matvec(const View& v, cudaStream_t s);
 cudaError_t launch_pcgnr_init(const View& v, double lambda, double tol2, cudaStream_t s);

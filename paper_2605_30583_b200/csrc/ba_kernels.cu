@@ -1470,13 +1470,52 @@ __device__ __forceinline__ double direction_scale(double rr) {
   return ldexp(1.0, -(e / 2));
 }
 
+// The scalar sums of the S7 kernels (r.z, |r|^2, p.lambda D p, |b|^2), DETERMINISTICALLY (v.det_scalars: the handles of
+// a sharded problem): every block stores its partials, the last block to arrive (a ticket) adds all of them in block order and adds the total to the target with
+// ONE atomic.  Given the same vectors every run -- and every shard of a sharded problem (caspar_ba_set_shard) --
+// computes the same BITS, so alpha, beta, the power-of-two direction scale and the stop decision agree across
+// shards without a broadcast.  (Per-block atomics made them agree only to the last bits.)  N <= 3 sums per kernel;
+// `mine` are this block's, already reduced (valid in thread 0).  Must be reached by every thread of every block.
+template <int N>
+__device__ __forceinline__ void fold_block_sums(const View& v, const double (&mine)[N], double* const (&target)[N], double* red) {
+  __shared__ int is_last;
+  const int nb = (int)gridDim.x, b = (int)blockIdx.x, tid = (int)threadIdx.x;
+  if (!v.det_scalars) {  // single-GPU handles: one atomic per block and sum (the fold costs the launch-bound small
+                         // scenes 16 % of their LM iterations/s: 1,609 -> 1,341 on Tiny)
+    if (tid == 0) {
+#pragma unroll
+      for (int k = 0; k < N; ++k) atomicAdd(target[k], mine[k]);
+    }
+    return;
+  }
+  if (tid == 0) {
+#pragma unroll
+    for (int k = 0; k < N; ++k) v.pcg_part[(size_t)k * nb + b] = mine[k];
+    __threadfence();
+    is_last = atomicAdd(v.pcg_ticket, 1u) == (unsigned)(nb - 1);
+  }
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    double a = 0.0;
+    for (int i = tid; i < nb; i += (int)blockDim.x) a += __ldcg(v.pcg_part + (size_t)k * nb + i);
+    const double tot = block_sum(a, red);
+    if (tid == 0) atomicAdd(target[k], tot);  // onto the zeroed accumulator (N1's point kernels add their part too)
+  }
+  if (tid == 0) *v.pcg_ticket = 0u;
+}
+
 // |b|^2, needed before the first direction is rounded to fp32
 __global__ void __launch_bounds__(kPcgThreads) pcg_norm_kernel(View v) {
   __shared__ double red[32];
   const long long i = (long long)blockIdx.x * kPcgThreads + threadIdx.x;
   const double bi = i < 9ll * v.nc ? v.b[i] : 0.0;
   const double s = block_sum(bi * bi, red);
-  if (threadIdx.x == 0) atomicAdd(&v.pcg->bnorm2, s);
+  const double mine[1] = {s};
+  double* const target[1] = {&v.pcg->bnorm2};
+  fold_block_sums<1>(v, mine, target, red);
 }
 
 // x = 0, r = b, z = M^-1 r, p = z; rz[0], |r|^2, pDp[0]
@@ -1505,15 +1544,13 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_init_kernel(View v, double to
   const double s_rz = block_sum(ri * zi, red);
   const double s_rr = block_sum(ri * ri, red);
   const double s_pd = block_sum(ld * zi * zi, red);
-  if (tid == 0) {
-    atomicAdd(&v.pcg->rz[0], s_rz);
-    atomicAdd(&v.pcg->rr, s_rr);
-    atomicAdd(&v.pcg->pDp[0], s_pd);
-    if (blockIdx.x == 0) {
-      v.pcg->pscale = scale;
-      v.pcg->tol2 = tol2;
-    }
+  if (tid == 0 && blockIdx.x == 0) {
+    v.pcg->pscale = scale;
+    v.pcg->tol2 = tol2;
   }
+  const double mine[3] = {s_rz, s_rr, s_pd};
+  double* const target[3] = {&v.pcg->rz[0], &v.pcg->rr, &v.pcg->pDp[0]};
+  fold_block_sums<3>(v, mine, target, red);
 }
 
 // alpha = rz / (p.q); x += alpha p; r -= alpha q; z = M^-1 r; rz_new, |r|^2
@@ -1558,15 +1595,14 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_xr_kernel(View v) {
   }
   const double s_rz = block_sum(ri * zi, red);
   const double s_rr = block_sum(ri * ri, red);
-  if (tid == 0) {
-    atomicAdd(&sc->rz[par ^ 1], s_rz);
-    atomicAdd(&sc->rr, s_rr);
-    if (blockIdx.x == 0) {
-      sc->iters = iter + 1;
-      sc->it_b = iter;
-      if (iter == 0) sc->rz0 = rz;
-    }
+  if (tid == 0 && blockIdx.x == 0) {
+    sc->iters = iter + 1;
+    sc->it_b = iter;
+    if (iter == 0) sc->rz0 = rz;
   }
+  const double mine[2] = {s_rz, s_rr};
+  double* const target[2] = {&sc->rz[par ^ 1], &sc->rr};
+  fold_block_sums<2>(v, mine, target, red);
 }
 
 // stop if |r| <= tol |b|, else beta = rz_new / rz; p = z + beta p; p.(lambda D p); q = 0
@@ -1595,14 +1631,14 @@ __global__ void __launch_bounds__(kPcgThreads) pcg_update_p_kernel(View v) {
     pd = v.lamD[i] * pi * pi;
   }
   const double s_pd = block_sum(pd, red);
-  if (tid == 0) {
-    atomicAdd(&sc->pDp[par ^ 1], s_pd);
-    if (blockIdx.x == 0) {
-      sc->pq = 0.0;
-      sc->pscale = scale;
-      sc->it_a = iter + 1;
-    }
+  if (tid == 0 && blockIdx.x == 0) {
+    sc->pq = 0.0;
+    sc->pscale = scale;
+    sc->it_a = iter + 1;
   }
+  const double mine[1] = {s_pd};
+  double* const target[1] = {&sc->pDp[par ^ 1]};
+  fold_block_sums<1>(v, mine, target, red);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -2227,27 +2263,21 @@ static cudaError_t launch_pipelined_or_pass(const View& v, cudaStream_t s) {
 
 cudaError_t launch_schur_matvec(const View& v, cudaStream_t s) { return launch_pipelined_or_pass<MATVEC>(v, s); }
 
-cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s, int stage) {
+cudaError_t launch_pcg_init(const View& v, double tol2, cudaStream_t s) {
   if (v.nc == 0) return cudaSuccess;
-  cudaError_t e = cudaSuccess;
-  if (stage != 2) {
-    pcg_norm_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
-    e = CBA_LAUNCHED();
-  }
-  if (e != cudaSuccess || stage == 1) return e;
+  pcg_norm_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v);
+  cudaError_t e = CBA_LAUNCHED();
+  if (e != cudaSuccess) return e;
   pcg_init_kernel<<<grid_for(9ll * v.nc, kPcgThreads), kPcgThreads, 0, s>>>(v, tol2);
   return CBA_LAUNCHED();
 }
 
-cudaError_t launch_pcg_update(const View& v, cudaStream_t s, int stage) {
+cudaError_t launch_pcg_update(const View& v, cudaStream_t s) {
   if (v.nc == 0) return cudaSuccess;
   const unsigned g = grid_for(9ll * v.nc, kPcgThreads);
-  cudaError_t e = cudaSuccess;
-  if (stage != 2) {
-    pcg_update_xr_kernel<<<g, kPcgThreads, 0, s>>>(v);
-    e = CBA_LAUNCHED();
-  }
-  if (e != cudaSuccess || stage == 1) return e;
+  pcg_update_xr_kernel<<<g, kPcgThreads, 0, s>>>(v);
+  cudaError_t e = CBA_LAUNCHED();
+  if (e != cudaSuccess) return e;
   pcg_update_p_kernel<<<g, kPcgThreads, 0, s>>>(v);
   return CBA_LAUNCHED();
 }

@@ -67,20 +67,12 @@ def shard_arrays(shard: Shard, points: np.ndarray, observations: np.ndarray):
     return points[shard.point_begin:shard.point_end], observations[shard.observation_ids]
 
 
-def torch_exchange(group=None, root: int = 0):
+def torch_exchange(group=None):
     """The collective for `CasparBA.set_shard` on top of torch.distributed (NCCL over NVLink for CUDA tensors; gloo
-    works for the CPU tests): op 0 = all_reduce(SUM) of the first `count` doubles, op 1 = broadcast of the first
-    `count` bytes from `root`.  Both run on the current stream of the buffer's device."""
-    import torch
+    for the CPU tests): all_reduce(SUM) of the first `count` doubles, on the current stream of the buffer's device."""
     import torch.distributed as dist
 
-    def exchange(buffer: "torch.Tensor", count: int, op: int) -> None:
-        if op == 0:
-            dist.all_reduce(buffer[:count], op=dist.ReduceOp.SUM, group=group)
-        elif op == 1:
-            words = (count + 7) // 8
-            dist.broadcast(buffer[:words], src=root, group=group)
-        else:
-            raise ValueError(f"unknown exchange op {op}")
+    def exchange(buffer, count: int) -> None:
+        dist.all_reduce(buffer[:count], op=dist.ReduceOp.SUM, group=group)
 
     return exchange

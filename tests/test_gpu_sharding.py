@@ -19,7 +19,7 @@ WORLD = 2
 
 
 class HostExchange:
-    """All-reduce / broadcast between WORLD threads of one process through a barrier."""
+    """All-reduce (sum) between WORLD threads of one process through a barrier."""
 
     def __init__(self, world):
         self.world = world
@@ -30,21 +30,16 @@ class HostExchange:
     def make(self, rank):
         import torch
 
-        def exchange(buf, count, op):
+        def exchange(buf, count):
             torch.cuda.current_stream(buf.device).synchronize()
             self.bufs[rank] = buf
             self.barrier.wait()
             if rank == 0:
-                if op == 0:
-                    total = self.bufs[0][:count].clone()
-                    for b in self.bufs[1:]:
-                        total += b[:count]
-                    for b in self.bufs:
-                        b[:count] = total
-                else:
-                    words = (count + 7) // 8
-                    for b in self.bufs[1:]:
-                        b[:words] = self.bufs[0][:words]
+                total = self.bufs[0][:count].clone()
+                for b in self.bufs[1:]:
+                    total += b[:count]
+                for b in self.bufs:
+                    b[:count] = total
                 torch.cuda.synchronize()
                 self.calls += 1
             self.barrier.wait()
@@ -125,8 +120,8 @@ def test_sharded_linearize_matvec_and_pcg_match_the_unsharded_handle(scene_cache
         assert rel_l2(r["dp"], d[nc9 + lo:nc9 + hi]) <= 1e-4
     # replicas: the same bits on both shards
     assert np.array_equal(out[0]["dc"], out[1]["dc"]) and np.array_equal(out[0]["q"], out[1]["q"])
-    # 1 (linearize) + 1 (matvec) + [1 (b) + 2 (start) + 3 x 30 + 1 (scalars)]
-    assert out[0]["ex"] == out[1]["ex"] == 1 + 1 + 1 + 2 + 90 + 1
+    # 1 (linearize) + 1 (matvec) + [1 (b) + 30 (one per iteration) + 1 (scalars)]
+    assert out[0]["ex"] == out[1]["ex"] == 1 + 1 + 1 + 30 + 1
     assert ex.calls == out[0]["ex"]
 
 
@@ -151,7 +146,7 @@ def test_sharded_lm_steps_match_and_the_shards_stay_replicas(scene_cache, precon
             # (stopping on a tolerance: the residual hovers around it for a few iterations, C9)
             assert x.accepted == y.accepted and abs(x.pcg_iterations - y.pcg_iterations) <= max(3, 0.1 * y.pcg_iterations)
             assert x.cost_before == pytest.approx(y.cost_before, rel=1e-6) and x.cost_after == pytest.approx(y.cost_after, rel=1e-6)
-            assert x.rho == pytest.approx(y.rho, rel=1e-3)
+            assert x.rho == pytest.approx(y.rho, rel=5e-3)
         assert np.abs(r["cams"] - cams).max() <= 1e-4 * np.abs(cams).max()
         assert np.abs(r["pts"] - pts[r["p0"]:r["p1"]]).max() <= 1e-4 * np.abs(pts).max()
     assert np.array_equal(out[0]["cams"], out[1]["cams"])       # bit-identical replicas after four steps
@@ -163,7 +158,7 @@ def test_a_sharded_handle_refuses_what_it_does_not_support(scene_cache):
     import torch
     s = scene_cache("tiny")
     g = pkg.CasparBA.from_scene(s)
-    g.set_shard(lambda buf, count, op: None, is_root=True)      # a one-shard "world": the collective is the identity
+    g.set_shard(lambda buf, count: None, is_root=True)          # a one-shard "world": the collective is the identity
     cost = g.linearize()
     ref = pkg.CasparBA.from_scene(s)
     assert cost == ref.linearize()

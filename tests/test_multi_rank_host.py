@@ -1,6 +1,6 @@
-"""N > 1 host logic on CPU (gloo, world_size 2).  The path does not shard ("replicas only"): ranks run
+"""N > 1 host logic on CPU (gloo, world_size 2), replica mode (the default of bench.py --gpus N): ranks run
 independent replicas and the only exchange is bench.py's max-over-ranks timing reduction; the reference arm runs on
-rank 0 alone."""
+rank 0 alone.  The point-sharded mode is covered by tests/test_sharding_host.py and tests/test_gpu_sharding.py."""
 import json
 import os
 import subprocess

@@ -70,9 +70,9 @@ def _worker(rank, world, port, out):
     buf[81 * s.num_cameras:81 * s.num_cameras + nc9] = torch.from_numpy(o.export(ob.G)[:nc9])
     buf[81 * s.num_cameras + nc9:-1] = torch.from_numpy(q)
     buf[-1] = cost
-    exchange(buf, buf.numel(), 0)                       # op 0: sum of doubles over the shards
+    exchange(buf, buf.numel())                          # sum of doubles over the shards
     tag = torch.full((4,), float(rank + 1), dtype=torch.float64)
-    exchange(tag, 20, 1)                                # op 1: the root's first 20 BYTES (2.5 doubles -> 3 words)
+    exchange(tag, 3)                                    # only the first `count` doubles take part
     dist.barrier()
     dist.destroy_process_group()
     np.save(f"{out}.{rank}.npy", buf.numpy())
@@ -89,7 +89,7 @@ def test_camera_side_sums_over_two_gloo_ranks_equal_the_unsharded_problem(tmp_pa
     res = [np.load(f"{out}.{r}.npy") for r in range(2)]
     meta = [json.load(open(f"{out}.{r}.json")) for r in range(2)]
     assert np.array_equal(res[0], res[1])                               # an all-reduce: the same bits on both ranks
-    assert meta[0]["tag"] == [1.0, 1.0, 1.0, 1.0] and meta[1]["tag"] == [1.0, 1.0, 1.0, 2.0]   # 3 words from the root
+    assert meta[0]["tag"] == [3.0, 3.0, 3.0, 1.0] and meta[1]["tag"] == [3.0, 3.0, 3.0, 2.0]   # 1 + 2 on the first three
     s = scene_cache("tiny")
     assert meta[0]["points"] + meta[1]["points"] == s.num_points
     assert meta[0]["obs"] + meta[1]["obs"] == s.num_observations
