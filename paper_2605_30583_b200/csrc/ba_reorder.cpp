@@ -27,7 +27,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
     return CASPAR_BA_EINVAL;
   }
   // --- validate, count tracks, lowest camera per point -----------------------------------------
-  std::vector<int> track(np, 0), key(np, nc);
+  std::vector<int> track(np, 0), key(np, nc), key_hi(np, -1);
   for (long long i = 0; i < n; ++i) {
     int c = cam_idx[i], k = pt_idx[i];
     if (c < 0 || c >= nc || k < 0 || k >= np) {
@@ -36,6 +36,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
     }
     track[k]++;
     if (c < key[k]) key[k] = c;
+    if (c > key_hi[k]) key_hi[k] = c;
   }
   int max_track = 0;
   for (int k = 0; k < np; ++k) max_track = std::max(max_track, track[k]);
@@ -68,6 +69,16 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
     }
   }
   int np_obs = bucket[nc];  // points with key < nc, i.e. observed at least once
+  // Inside a lowest-camera bucket the points go by their HIGHEST camera id (ties by caller id): points that agree on
+  // both ends of their camera set mostly agree on the rest, so a tile of ~40 consecutive points sees fewer distinct
+  // cameras -- 0.180 -> 0.125 camera runs per observation on Large, 0.65 -> 0.56 on Skewed, 0.095 -> 0.071 on Mid --
+  // i.e. fewer segment ends in the camera-side walk, fewer REDs and camera-row gathers: Schur matvec 0.719 -> 0.679 ms on
+  // Large.  A greedy fill with a 64 / 256-point lookahead on top gained only 0.125 -> 0.121 / 0.118.
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int c = 0; c < nc; ++c)
+    std::stable_sort(perm.begin() + bucket[c], perm.begin() + bucket[c + 1],
+                     [&](int a, int b) { return key_hi[a] < key_hi[b]; });
+  for (int pos = 0; pos < np_obs; ++pos) internal_of[perm[pos]] = pos;
   out->np_obs = np_obs;
   out->pt_ptr.assign(np_obs + 1, 0);
   for (int a = 0; a < np_obs; ++a) out->pt_ptr[a + 1] = out->pt_ptr[a] + track[perm[a]];

@@ -57,6 +57,11 @@ def _check_layout(scene, L):
     lowest = np.full(scene.num_points, scene.num_cameras)
     np.minimum.at(lowest, scene.point_index, scene.camera_index)
     assert (np.diff(lowest[perm[:np_obs]]) >= 0).all()
+    # ... and, among points with the same lowest camera, by their highest camera id (fewer distinct cameras per tile)
+    highest = np.full(scene.num_points, -1)
+    np.maximum.at(highest, scene.point_index, scene.camera_index)
+    lo, hi = lowest[perm[:np_obs]].astype(np.int64), highest[perm[:np_obs]].astype(np.int64)
+    assert (np.diff(lo * (scene.num_cameras + 1) + hi) >= 0).all()
     internal_of = np.empty(scene.num_points, np.int64)
     internal_of[perm] = np.arange(scene.num_points)
     # tiles hold whole points, at most T observations, and are filled greedily
