@@ -2161,9 +2161,23 @@ cudaError_t launch_prepare_blocks(const View& v, double lambda, int precondition
   return e;
 }
 
+// A handle without observations (an empty shard of a sharded problem) still runs the PCG vector kernels on the summed
+// b and q: the accumulators that the matvec kernel zeroes for the update that follows it must be zeroed all the same.
+__global__ void pcg_zero_accumulators_kernel(View v) {
+  if (v.pcg->done) return;
+  const int nxt = (v.pcg->it_a + 1) & 1;
+  v.pcg->rz[nxt] = 0.0;
+  v.pcg->pDp[nxt] = 0.0;
+  v.pcg->rr = 0.0;
+}
+
 template <int MODE>
 static cudaError_t launch_pass(const View& v, cudaStream_t s) {
-  if (v.num_tiles == 0) return cudaSuccess;
+  if (v.num_tiles == 0) {
+    if (MODE != MATVEC || v.nc == 0) return cudaSuccess;
+    pcg_zero_accumulators_kernel<<<1, 1, 0, s>>>(v);
+    return CBA_LAUNCHED();
+  }
   switch (v.T) {
     case 128: schur_pass_kernel<128, MODE><<<v.num_tiles, 128, 0, s>>>(v); break;
     case 192: schur_pass_kernel<192, MODE><<<v.num_tiles, 192, 0, s>>>(v); break;
@@ -2250,7 +2264,7 @@ static void pipelined_launch(const View& v, const PipeLayout& L, int grid, cudaS
 // carry the g_p rows, the ring still has a stage to spare), else through the one-block-per-tile pass.
 template <int MODE>
 static cudaError_t launch_pipelined_or_pass(const View& v, cudaStream_t s) {
-  if (!pipelined_matvec_available(v)) return launch_pass<MODE>(v, s);
+  if (!pipelined_matvec_available(v) || v.num_tiles == 0) return launch_pass<MODE>(v, s);
   const int NG = pipe_groups(v.T);
   const PipeLayout L = pipe_layout(v.T, NG, v.max_pts_per_tile, v.meta_max_bytes, v.num_hot, smem_optin(), MODE != MATVEC);
   if (L.stages < NG + 1) return launch_pass<MODE>(v, s);

@@ -23,7 +23,7 @@ class HostExchange:
 
     def __init__(self, world):
         self.world = world
-        self.barrier = threading.Barrier(world, timeout=120)
+        self.barrier = threading.Barrier(world, timeout=30)
         self.bufs = [None] * world
         self.calls = 0
 
@@ -173,4 +173,51 @@ def test_a_sharded_handle_refuses_what_it_does_not_support(scene_cache):
     d = ref.lm_step(LAM, 1e-6, 50, 0)
     assert c.cost_after == pytest.approx(d.cost_after, rel=1e-7)
     g.close()
+    ref.close()
+
+
+def test_an_empty_shard_takes_part_in_every_exchange(scene_cache):
+    """More ranks than work: a shard with no points and no observations still replicates the cameras, makes the same
+    calls and contributes zeros; the other shard then reproduces the unsharded problem and both end with the same
+    cameras."""
+    import torch
+    s = scene_cache("tiny")
+    ex = HostExchange(WORLD)
+    out, err = [None] * WORLD, [None] * WORLD
+
+    def work(rank):
+        try:
+            torch.cuda.set_device(0)
+            with torch.cuda.stream(torch.cuda.Stream()):
+                if rank == 0:
+                    g = pkg.CasparBA.from_scene(s)
+                else:
+                    g = pkg.CasparBA(s.cameras, np.zeros((0, 3), np.float32), np.zeros((0, 2), np.float32),
+                                     np.zeros(0, np.int32), np.zeros(0, np.int32))
+                g.set_shard(ex.make(rank), is_root=(rank == 0))
+                steps = [g.lm_step(LAM, 1e-6, 50, 0) for _ in range(3)]
+                out[rank] = (steps, g.cameras.cpu().numpy(), g.stats().shard_exchanges)
+                g.close()
+        except BaseException as e:  # noqa: BLE001
+            err[rank] = e
+            ex.barrier.abort()
+
+    threads = [threading.Thread(target=work, args=(r,)) for r in range(WORLD)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    for e in err:
+        if e is not None and not isinstance(e, threading.BrokenBarrierError):
+            raise e
+    assert not any(err)
+    ref = pkg.CasparBA.from_scene(s)
+    want = [ref.lm_step(LAM, 1e-6, 50, 0) for _ in range(3)]
+    for x, y, z in zip(out[0][0], out[1][0], want):
+        assert x.accepted == y.accepted == z.accepted and x.pcg_iterations == y.pcg_iterations
+        assert x.cost_after == y.cost_after                                  # the two shards: the same bits
+        assert x.cost_after == pytest.approx(z.cost_after, rel=1e-7) and abs(x.pcg_iterations - z.pcg_iterations) <= 3
+    assert np.array_equal(out[0][1], out[1][1])
+    assert np.abs(out[0][1] - ref.cameras.cpu().numpy()).max() <= 1e-5 * np.abs(out[0][1]).max()
+    assert out[0][2] == out[1][2]
     ref.close()
