@@ -232,14 +232,14 @@ def test_fusion_survives_a_parameter_reset_and_the_graph_chunks(scene_cache):
     b = [ref.lm_step(LAM, 1e-6, s.pcg_max_iter, 0) for _ in range(3)]
     for x, y in zip(a, b):
         assert x.accepted and y.accepted and x.pcg_iterations == y.pcg_iterations
-        assert x.cost_after == pytest.approx(y.cost_after, rel=1e-7)
+        assert x.cost_after == pytest.approx(y.cost_after, rel=1e-6)
     cam_h = torch.from_numpy(s.cameras.copy()).pin_memory()
     pts_h = torch.from_numpy(s.points.copy()).pin_memory()
     g.set_parameters_host(cam_h, pts_h)
     ref.set_parameters_host(cam_h, pts_h)
     x, y = g.lm_step(LAM, 1e-6, s.pcg_max_iter, 0), ref.lm_step(LAM, 1e-6, s.pcg_max_iter, 0)
     assert x.pcg_iterations == y.pcg_iterations
-    assert x.cost_before == pytest.approx(y.cost_before, rel=1e-12) and x.cost_after == pytest.approx(y.cost_after, rel=1e-7)
+    assert x.cost_before == pytest.approx(y.cost_before, rel=1e-12) and x.cost_after == pytest.approx(y.cost_after, rel=1e-6)
     assert x.cost_before == pytest.approx(b[0].cost_before, rel=1e-12)
     g.close()
     ref.close()
