@@ -14,7 +14,6 @@ from oracle import binding as ob
 pytestmark = pytest.mark.gpu
 
 LAM = float(np.float32(1e-2))
-D_MIN = 1e-6
 
 
 def rel_l2(a, b):
@@ -119,44 +118,18 @@ def test_sampled_camera_and_point_blocks(large):
     assert rel_l2(gp_g, gp_o) <= 1e-4
 
 
-def _schur_row(large, j, p, lam):
-    """(S p)_j from the definition: lambda D_j p_j + sum_{i in j} J_c^T (u_i - J_p s_k(i)),
-    s_k = V'_k^-1 sum_{i' in k} J_p^T J_c p_j(i'), V'_k = V_k + lambda max(diag V_k, d_min),
-    D_j = max(diag U_j, d_min).  Every number comes from the oracle's per-observation routine."""
-    s, lin = large["scene"], large["lin"]
-    mine = large["by_cam"][large["cam_ptr"][j]:large["cam_ptr"][j + 1]]
-    u_diag = sum((lin(i)[1] ** 2).sum(axis=0) for i in mine)
-    q = lam * np.maximum(u_diag, D_MIN) * p[j]
-    for i in mine:
-        k = s.point_index[i]
-        v, t = np.zeros((3, 3)), np.zeros(3)
-        for i2 in large["by_pt"][large["pt_ptr"][k]:large["pt_ptr"][k + 1]]:
-            _, jc2, jp2 = lin(i2)
-            v += jp2.T @ jp2
-            t += jp2.T @ (jc2 @ p[s.camera_index[i2]])
-        v += lam * np.diag(np.maximum(np.diag(v), D_MIN))
-        _, jc, jp = lin(i)
-        q += jc.T @ (jc @ p[j] - jp @ np.linalg.solve(v, t))
-    return q
-
-
-def test_sampled_schur_matvec_rows_and_operator_properties(large):
+def test_schur_operator_properties_at_full_size(large):
+    """Any size: S is symmetric and positive definite.  (The rows of q = S p themselves are compared with the ORACLE's
+    at full size in tests/test_gpu_golden.py; the numpy restatement of the operator that used to live here is gone.)"""
     s, g = large["scene"], large["gpu"]
     rng = np.random.default_rng(29)
     n = 9 * s.num_cameras
     x = rng.normal(size=n).astype(np.float32).astype(np.float64)
     y = rng.normal(size=n).astype(np.float32).astype(np.float64)
     sx, sy = g.schur_matvec(LAM, x), g.schur_matvec(LAM, y)
-    # any size: symmetric, positive definite
     a, b = float(y @ sx), float(x @ sy)
     assert abs(a - b) <= 1e-4 * max(abs(a), abs(b))
     assert float(x @ sx) > 0 and float(y @ sy) > 0
-    # sampled rows against the definition
-    xs = x.reshape(-1, 9)
-    for j in rng.integers(0, s.num_cameras, 3):
-        want = _schur_row(large, int(j), xs, LAM)
-        got = sx.reshape(-1, 9)[j]
-        assert np.linalg.norm(got - want) <= 1e-4 * np.linalg.norm(want), (j, got, want)
 
 
 def test_one_lm_iteration_at_full_size(large):
