@@ -169,3 +169,71 @@ def test_layout_errors_carry_their_text():
     with pytest.raises(pkg.CasparError) as e:
         pkg.plan_layout(s.num_cameras, s.num_points, bad, s.point_index)
     assert e.value.code == -1 and "out of range at observation 17" in str(e.value)
+
+
+def test_ranks_are_bank_aware(scene_cache):
+    """S0 chooses WHICH position of its point's rank range a slot takes so that the 16 slots of a half-warp scatter to
+    distinct 8-byte shared-memory banks (rank mod 16) where possible.  Against ranks in plain point-major
+    input order the number of colliding slots must drop by more than half."""
+    s = scene_cache("mid", grid=(10, 12), num_points=40_000)
+    L = pkg.plan_layout(s.num_cameras, s.num_points, s.camera_index, s.point_index)
+    T, obs, rank = L["T"], L["obs_of_slot"], L["rank"].astype(np.int64)
+    perm = L["pt_perm"]
+    internal_of = np.empty(s.num_points, np.int64)
+    internal_of[perm] = np.arange(s.num_points)
+    pt_ptr = L["pt_ptr"].astype(np.int64)
+
+    def collisions(r, valid):
+        """slots whose bank is already taken by an earlier slot of the same half-warp"""
+        total = 0
+        for h in range(0, r.size, 16):
+            v = valid[h:h + 16]
+            banks = (r[h:h + 16][v]) & 15
+            total += banks.size - np.unique(banks).size
+        return total
+
+    got = naive = 0
+    for t in range(L["num_tiles"]):
+        sl = slice(t * T, (t + 1) * T)
+        o, valid = obs[sl], obs[sl] >= 0
+        base = pt_ptr[L["tile_pt"][t]]
+        k = internal_of[s.point_index[np.where(valid, o, 0)]]
+        # plain point-major input order: a slot's position inside its point = how many of the point's observations
+        # have a smaller caller index
+        order = np.lexsort((np.where(valid, o, 0), k))
+        pos = np.empty(T, np.int64)
+        ks, os_ = k[order], o[order]
+        first = np.r_[True, ks[1:] != ks[:-1]]
+        start = np.maximum.accumulate(np.where(first, np.arange(T), 0))
+        pos[order] = np.arange(T) - start
+        r_naive = pt_ptr[k] - base + pos
+        got += collisions(rank[sl], valid)
+        naive += collisions(r_naive, valid)
+    assert naive > 0 and got < 0.5 * naive, (got, naive)
+
+
+def test_point_order_keeps_cameras_together(scene_cache):
+    """Points go by (lowest, highest) camera id: a tile of consecutive points then sees fewer distinct cameras than with
+    the lowest camera id alone (0.180 -> 0.125 camera runs per observation on the full Large scene)."""
+    s = scene_cache("large", grid=(24, 32), num_points=60_000)
+    L = pkg.plan_layout(s.num_cameras, s.num_points, s.camera_index, s.point_index)
+    runs_per_obs = L["camera_runs"] / s.num_observations
+    # the same tiling with points ordered by lowest camera only (ties by caller id), in numpy
+    lowest = np.full(s.num_points, s.num_cameras)
+    np.minimum.at(lowest, s.point_index, s.camera_index)
+    order = np.argsort(lowest, kind="stable")
+    track = np.bincount(s.point_index, minlength=s.num_points)
+    by_pt = np.argsort(s.point_index, kind="stable")
+    ptr = np.concatenate([[0], np.cumsum(track)])
+    runs, used, cams = 0, 0, set()
+    for kpt in order:
+        if track[kpt] == 0:
+            continue
+        if used + track[kpt] > L["T"]:
+            runs += len(cams)
+            used, cams = 0, set()
+        used += track[kpt]
+        cams.update(s.camera_index[by_pt[ptr[kpt]:ptr[kpt + 1]]].tolist())
+    runs += len(cams)
+    # (this shrunken scene has 78 points per camera, the full one 328: the gain here is 14 %, there 31 %)
+    assert runs_per_obs < 0.92 * runs / s.num_observations, (runs_per_obs, runs / s.num_observations)
