@@ -93,9 +93,9 @@ typedef struct {
 
 /* PAPER.md:167 (one device memory block, all arrays views into it), :137-149 (block-local sorted index built once
  * and reused: here the tile layout) -- step S0.
- * Build a solver for one problem on the CURRENT device: validates the indices (on the host, in the pass that
- * counts the tracks: S0 runs there), reorders the observations (sorted by point into tiles of whole points,
- * camera runs contiguous inside a tile), carves the arena.  Every later call on the handle runs on that device
+ * Build a solver for one problem on the CURRENT device: validates the indices (on the device when the index arrays
+ * live there, else on the host in the pass that counts the tracks), reorders the observations (S0, on the host:
+ * sorted by point into tiles of whole points, camera runs contiguous inside a tile), carves the arena.  Every later call on the handle runs on that device
  * whatever device is current in the calling thread.
  * Errors: EINVAL (bad sizes / indices / a track longer than CASPAR_BA_MAX_TRACK / CASPAR_BA_TILE not one of the
  * supported sizes), ENOMEM, ECUDA; the text is available from caspar_ba_last_error(NULL). */

@@ -499,8 +499,32 @@ static int create_impl(const caspar_ba_problem* pb, void* cuda_stream, caspar_ba
     return bail(e == cudaErrorMemoryAllocation ? CASPAR_BA_ENOMEM : CASPAR_BA_ECUDA,
                 std::string(where) + ": " + cudaGetErrorString(e));
   };
-  // S0 runs on the host, so the indices come to the host (the source may be device or host memory) and are
-  // validated there, in the same pass that counts the tracks.
+  // Index arrays that live on the DEVICE are validated there first: a bad index is reported without
+  // moving 8 bytes per observation to the host.
+  if (n > 0) {
+    cudaPointerAttributes ac{}, ap{};
+    const bool dev_c = cudaPointerGetAttributes(&ac, pb->camera_index) == cudaSuccess &&
+                       (ac.type == cudaMemoryTypeDevice || ac.type == cudaMemoryTypeManaged);
+    const bool dev_p = cudaPointerGetAttributes(&ap, pb->point_index) == cudaSuccess &&
+                       (ap.type == cudaMemoryTypeDevice || ap.type == cudaMemoryTypeManaged);
+    cudaGetLastError();
+    if (dev_c && dev_p) {
+      unsigned long long* flag = nullptr;
+      unsigned long long bad = ~0ull;
+      cudaError_t e = cudaMalloc(&flag, sizeof(unsigned long long));
+      if (e == cudaSuccess) e = cudaMemcpyAsync(flag, &bad, sizeof bad, cudaMemcpyHostToDevice, s);
+      if (e == cudaSuccess) e = launch_validate_indices(pb->camera_index, pb->point_index, n, pb->num_cameras, pb->num_points, flag, s);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, flag, sizeof bad, cudaMemcpyDeviceToHost, s);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+      if (flag) cudaFree(flag);
+      take_launch_count();
+      if (e != cudaSuccess) return cuda_bail(e, "validation of the index arrays");
+      if (bad != ~0ull)
+        return bail(CASPAR_BA_EINVAL, "camera_index / point_index out of range at observation " + std::to_string(bad) + " (validated on the device)");
+    }
+  }
+  // S0 runs on the host, so the indices come to the host (the source may be device or host memory; host arrays are
+  // validated there, in the same pass that counts the tracks).
   std::vector<int> cam_idx((size_t)n), pt_idx((size_t)n);
   if (n > 0) {
     cudaError_t e = cudaMemcpy(cam_idx.data(), pb->camera_index, sizeof(int) * (size_t)n, cudaMemcpyDefault);

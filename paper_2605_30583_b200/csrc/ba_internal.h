@@ -181,6 +181,8 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
                          Reordered* out, std::string* err);
 
 // ---- kernel launchers (ba_kernels.cu); all enqueue on `s` and return the launch status ----
+cudaError_t launch_validate_indices(const int* cam_idx_dev, const int* pt_idx_dev, long long n, int nc, int np,
+                                    unsigned long long* first_bad_dev, cudaStream_t s);
 cudaError_t launch_gather_observations(const View& v, const float* observations, float2* px_out, cudaStream_t s);
 cudaError_t launch_pack_points(const View& v, const float* points_caller, float4* dst, cudaStream_t s);
 cudaError_t launch_unpack_points(const View& v, const float4* src, float* points_caller, cudaStream_t s);

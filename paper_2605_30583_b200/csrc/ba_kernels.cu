@@ -2038,6 +2038,26 @@ __global__ void matvec_finish_kernel(View v, double* __restrict__ q_out) {
 // ------------------------------------------------------------------------------------------------
 static inline unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
 
+// "index out of range -- validated on device at create".  first_bad receives the lowest offending
+// observation index (or stays at its initial value).
+__global__ void validate_indices_kernel(const int* __restrict__ cam_idx, const int* __restrict__ pt_idx, long long n,
+                                        int nc, int np, unsigned long long* __restrict__ first_bad) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (; i < n; i += stride) {
+    const int c = cam_idx[i], k = pt_idx[i];
+    if (c < 0 || c >= nc || k < 0 || k >= np) atomicMin(first_bad, (unsigned long long)i);
+  }
+}
+
+cudaError_t launch_validate_indices(const int* cam_idx_dev, const int* pt_idx_dev, long long n, int nc, int np,
+                                    unsigned long long* first_bad_dev, cudaStream_t s) {
+  if (n == 0) return cudaSuccess;
+  const long long blocks = (n + 255) / 256;
+  validate_indices_kernel<<<(unsigned)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, s>>>(cam_idx_dev, pt_idx_dev, n, nc, np, first_bad_dev);
+  return CBA_LAUNCHED();
+}
+
 cudaError_t launch_gather_observations(const View& v, const float* observations, float2* px_out, cudaStream_t s) {
   if (v.n_slots == 0) return cudaSuccess;
   gather_observations_kernel<<<grid_for(v.n_slots, 256), 256, 0, s>>>(v, observations, px_out);

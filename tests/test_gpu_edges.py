@@ -45,9 +45,15 @@ def test_empty_problems():
 
 def test_error_codes():
     one9, one3 = np.zeros((1, 9), np.float32), np.zeros((1, 3), np.float32)
-    with pytest.raises(pkg.CasparError) as e:      # index out of range
+    with pytest.raises(pkg.CasparError) as e:      # index out of range (the binding hands DEVICE index arrays over)
         pkg.CasparBA(one9, one3, np.zeros((1, 2), np.float32), np.array([1], np.int32), np.array([0], np.int32))
-    assert e.value.code == -1
+    assert e.value.code == -1 and "observation 0 (validated on the device)" in str(e.value)
+    ci = np.zeros(5000, np.int32)
+    pi = np.zeros(5000, np.int32)
+    pi[[4321, 777]] = 9                            # the LOWEST offending observation is reported
+    with pytest.raises(pkg.CasparError) as e:
+        pkg.CasparBA(one9, one3, np.zeros((5000, 2), np.float32), ci, pi)
+    assert e.value.code == -1 and "observation 777 (validated on the device)" in str(e.value)
     with pytest.raises(pkg.CasparError) as e:      # negative index
         pkg.CasparBA(one9, one3, np.zeros((1, 2), np.float32), np.array([0], np.int32), np.array([-1], np.int32))
     assert e.value.code == -1
