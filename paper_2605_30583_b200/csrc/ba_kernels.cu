@@ -1108,11 +1108,11 @@ __global__ void __launch_bounds__(T, blocks_per_sm(T)) schur_pass_kernel(View v)
 // long-scoreboard stalls at 39 % of HBM peak (history).
 // ------------------------------------------------------------------------------------------------
 struct PipeLayout {  // byte offsets inside one stage / inside the dynamic shared memory
-  int j, cam, rank, vinv, gp, meta, stage_bytes;
+  int j, cam, rank, vinv, gp, meta, stage_bytes, sbuf_stride;
   int stages, groups, tbuf, tbuf_bytes, sbuf, sbuf_bytes, scratch, hot, bars, total;
 };
 
-constexpr int kWarpScratchBytes = 1408;  // per consumer warp: 9 x 33 floats of products + 32 camera ids
+constexpr int kWarpScratchBytes = 1328;  // per consumer warp: 9 x 33 floats of products + 32 camera ids (1,316 B)
 
 // NG consumer groups of T threads share the ring; each group owns a staging area for the point-side sums
 // t_k (by rank) and one for the per-point results s_k (by local point id).
@@ -1130,7 +1130,11 @@ __host__ __device__ inline PipeLayout pipe_layout(int T, int NG, int max_pts, in
   L.meta = with_gp ? up(L.gp + max_pts * 16) : L.gp;
   L.stage_bytes = up(L.meta + meta_max);
   L.tbuf_bytes = up(3 * (T + 2) * 8);  // the point side is carried in fp64 (see schur_pass_kernel)
-  L.sbuf_bytes = up(3 * (T + 5) * 8);
+  // sbuf is indexed by POINT (<= max_pts), not by slot; row stride = 5 mod 16: the 15 storing lanes of phase B (point
+  // lp = 0..4, component c) hit 64-bit banks lp + 5 c.  (Shared memory is what limits the ring: the fp64 point side cut
+  // it from 6 to 4 stages on Large; the slimmer sbuf and scratch buy a 5th back: 0.672 -> 0.665 ms.)
+  L.sbuf_stride = ((max_pts + 15) & ~15) + 5;
+  L.sbuf_bytes = up(3 * L.sbuf_stride * 8);
   const int hot_bytes = up(num_hot * 9 * 8);  // per-CTA fp64 accumulators of the hot cameras' q rows
   const int fixed = NG * (L.tbuf_bytes + L.sbuf_bytes) + NG * (T / 32) * kWarpScratchBytes + hot_bytes + 256;
   int st = (smem_limit - fixed) / L.stage_bytes;
@@ -1219,8 +1223,8 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
   const int bar_id = 1 + g;
   // row stride T + 2: the six lanes of a point in phase B (component c, half h) read banks 2c + h + rank: distinct
   double(*tbuf)[T + 2] = reinterpret_cast<double(*)[T + 2]>(smem + L.tbuf + (size_t)g * L.tbuf_bytes);  // by rank
-  // row stride T + 5: the 15 storing lanes of phase B (point lp = 0..4, component c) hit 64-bit banks lp + 5 c: distinct
-  double(*sbuf)[T + 5] = reinterpret_cast<double(*)[T + 5]>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // by point
+  double* sbuf = reinterpret_cast<double*>(smem + L.sbuf + (size_t)g * L.sbuf_bytes);  // [3][sbuf_stride], by point
+  const int sstride = L.sbuf_stride;
   float* rows = reinterpret_cast<float*>(smem + L.scratch + (size_t)(tid >> 5) * kWarpScratchBytes);
   int* camrow = reinterpret_cast<int*>(rows + 9 * 33);
   // p.q = sum_i u_i.e_i (+ p.lambda D_c p, added by the update kernel): the curvature of the operator AS COMPUTED,
@@ -1320,7 +1324,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
             reinterpret_cast<float*>(v.dp + reinterpret_cast<const int*>(st + L.meta)[3] + k)[c] = (float)sc;
             dg_part += sc * gc;
           }
-          sbuf[c][k] = sc;
+          sbuf[c * sstride + k] = sc;
         }
       }
     }
@@ -1333,7 +1337,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         const float4 x4 = reinterpret_cast<const float4*>(st + L.j + 4 * T * 16)[gt];  // Jc16 Jc17 Jp0 Jp1
         const float4 x5 = reinterpret_cast<const float4*>(st + L.j + 5 * T * 16)[gt];  // Jp2 .. Jp5
         const double u0 = (double)uf0, u1 = (double)uf1;
-        const double s0 = sbuf[0][pid], s1 = sbuf[1][pid], s2 = sbuf[2][pid];
+        const double s0 = sbuf[pid], s1 = sbuf[sstride + pid], s2 = sbuf[2 * sstride + pid];
         const double w0 = (double)x4.z * s0 + (double)x4.w * s1 + (double)x5.x * s2;  // J_p s_k
         const double w1 = (double)x5.y * s0 + (double)x5.z * s1 + (double)x5.w * s2;
         if (MODE == BACKSUB) {  // |J delta|^2 of this observation
