@@ -40,3 +40,27 @@ def scaled_block_rel(u_gpu, u_ref) -> np.ndarray:
     num = np.linalg.norm((u_gpu - u_ref) / s, axis=(1, 2))
     den = np.linalg.norm(u_ref / s, axis=(1, 2))
     return num / den
+
+
+# ---- cameras along a replayed LM schedule (C16) -------------------------------------------------------
+# Once a schedule has converged (model decrease below 1e-6 of the cost: the replay tests already treat such a step's
+# right-hand side as fp32 rounding noise), delta = S^-1 b is that noise divided by a damping that keeps shrinking,
+# and it lands in the directions the data does not fix (the similarity gauge of a bundle-adjustment problem, held by
+# lambda D alone).  The cost does not see it (matched to 1e-11 there); the cameras drift run to run -- measured on
+# Small over repeated runs of the same binary: 2e-5 ... 1.5e-4 on w and t after steps 9-11 at lambda 5e-7 ... 6e-8,
+# against 3e-8 after the last significant step.  So the cameras are gated at 1e-4 after every SIGNIFICANT step,
+# and the end point of the noise tail at TAIL_CAMERA_TOL.
+SIGNIFICANT_STEP = 1e-6
+TAIL_CAMERA_TOL = 1e-3
+
+
+def significant_step(st) -> bool:
+    """`st`: the ORACLE's record of the step."""
+    return bool(st.accepted) and st.model_decrease > SIGNIFICANT_STEP * st.cost_before
+
+
+def assert_cameras_match(gpu_cameras, oracle_cameras, tol: float, what=""):
+    cams = gpu_cameras.detach().cpu().numpy().astype(np.float64) if hasattr(gpu_cameras, "detach") else gpu_cameras
+    ref = np.asarray(oracle_cameras, np.float64)
+    assert np.abs(cams - ref).max() <= tol * np.abs(ref).max(), what
+    return assert_per_class(cams, ref, tol, what)

@@ -13,7 +13,8 @@ import pytest
 import oracle
 import paper_2605_30583_b200 as pkg
 from oracle import binding as ob
-from parity_util import assert_per_class, per_class_rel_l2, rel_l2, scaled_block_rel
+from parity_util import (TAIL_CAMERA_TOL, assert_cameras_match, assert_per_class, per_class_rel_l2, rel_l2,
+                         scaled_block_rel, significant_step)
 
 pytestmark = pytest.mark.gpu
 
@@ -57,19 +58,28 @@ def test_pose3_linearize_parity(scene_cache, key, eps):
 @pytest.mark.parametrize("key", ["tiny", "small", "large"])
 def test_pose3_lm_schedule_parity(scene_cache, key):
     """The oracle's adaptive run with the Pose3 camera, replayed on the GPU: cost at every step to 1e-4, and the
-    cameras after the run (accepted steps RETRACT the rotation: w <- Log(Exp(w) Exp(d_w)))."""
+    cameras after every significant step (accepted steps RETRACT the rotation: w <- Log(Exp(w) Exp(d_w)))."""
     name, kw = SCENES[key]
     s = scene_cache(name, **kw)
     eps = 1e-6
     o = oracle.OracleBA.from_scene(s, camera_model=1, depth_epsilon=eps)
     ref = o.solve(s.lm_iterations, 1e-2, 1e-10, s.pcg_max_iter)
+    o.close()
+    o = oracle.OracleBA.from_scene(s, camera_model=1, depth_epsilon=eps)   # the same run again, step by step
     g = pkg.CasparBA.from_scene(s, camera_model=1, depth_epsilon=eps)
+    resolved = True
     for t, st in enumerate(ref):
-        got = g.lm_step(float(np.float32(st.lam)), 1e-10, s.pcg_max_iter, accept_mode=1 if st.accepted else 2)
+        mode = 1 if st.accepted else 2
+        got = g.lm_step(float(np.float32(st.lam)), 1e-10, s.pcg_max_iter, accept_mode=mode)
+        o.lm_step(st.lam, 1e-10, s.pcg_max_iter, accept_mode=mode)
         assert abs(got.cost_before - st.cost_before) <= 1e-4 * st.cost_before, t
         assert abs(got.cost_after - st.cost_after) <= 1e-4 * st.cost_after, t
-    cams = g.cameras.cpu().numpy().astype(np.float64)
-    assert max(per_class_rel_l2(cams, o.cameras).values()) <= 1e-4
+        resolved &= st.pcg_rel_residual <= 1e-2
+        # C16: 1e-4 per class after every significant step; the converged tail only drifts along the gauge
+        if resolved and significant_step(st):
+            assert_cameras_match(g.cameras, o.cameras, 1e-4, ("cameras after step", t))
+    if resolved:
+        assert_cameras_match(g.cameras, o.cameras, TAIL_CAMERA_TOL, "final cameras")
     g.close()
     o.close()
 
