@@ -188,6 +188,28 @@ int caspar_ba_set_shard(caspar_ba_t* h, caspar_ba_exchange_fn fn, void* ctx, dou
  * step S9 without the update: F at the caller's current parameters.  cost_out: HOST, required. */
 int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out);
 
+/* PAPER.md:194-203 (residual only) -- step S9 for callers that cannot allocate (code under CUDA-graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): F = 1/2 sum rho(|r_i|^2) at the parameters in `problem`, with NO handle
+ * and NO allocation.  The scratch the handle path keeps in its arena (the S1 camera table, the per-block partial
+ * sums) is a fixed device array inside the library: 144 B x CASPAR_BA_STATIC_MAX_CAMERAS + 4.6 KiB = 2.25 MiB, held
+ * by every GPU that loads the library until the process exits.
+ *   problem: num_cameras <= CASPAR_BA_STATIC_MAX_CAMERAS; cameras, points, observations, camera_index, point_index
+ *            are ALL DEVICE pointers on the CURRENT device (read only, caller's order; nothing is copied or kept);
+ *            robust_loss / robust_scale / depth_epsilon as in caspar_ba_create; damping_mode and camera_model do not
+ *            enter the cost and are ignored.
+ *   cost_out_dev: DEVICE double, written by the last of the three kernels the call enqueues on `cuda_stream`.
+ * Asynchronous: no synchronisation, no host result; calls cudaMalloc / cudaFree or any allocating routine never.
+ * An index out of range cannot be reported without a round trip: it makes *cost_out_dev NaN (no fault).
+ * ALL calls on one GPU share the scratch array: calls that overlap there (two streams, two host threads) race.  A
+ * call writes every scratch word before it reads it, so nothing has to be cleared and the previous call's contents
+ * never show.  The first call on a device resolves the array's address (and, with lazy module loading, loads the
+ * kernels): make one call outside stream capture first.
+ * Errors: EINVAL (null pointer, negative size, num_cameras > CASPAR_BA_STATIC_MAX_CAMERAS, robust_scale <= 0 with
+ * robust_loss = 1, a pointer that is not device memory of the current device), ECUDA; the text is available from
+ * caspar_ba_last_error(NULL). */
+#define CASPAR_BA_STATIC_MAX_CAMERAS 16384
+int caspar_ba_cost_static(const caspar_ba_problem* problem, double* cost_out_dev, void* cuda_stream);
+
 /* frees the one arena (and the handle's events, graph, pinned scalars).  NULL is a no-op. */
 void caspar_ba_destroy(caspar_ba_t* h);
 

@@ -6,7 +6,7 @@ point-eliminated (Schur) normal equations.  The product is the C-ABI library
 `libcaspar_ba.so` (include/caspar_ba.h, csrc/); this package only marshals arguments to it.
 """
 from .binding import (CasparBA, CasparError, PcgInfo, Stats, Step, StepInfo, EXPORTED_SYMBOLS,  # noqa: F401
-                      load_library, library_path, plan_layout)
+                      load_library, library_path, plan_layout, cost_static, STATIC_MAX_CAMERAS)
 from .binding import RESIDUALS, JC, JP, U, V, G, SCHUR_RHS, DELTA, PRECONDITIONER  # noqa: F401
 from .binding import OK, EINVAL, ECUDA, ENOMEM, ENUMERIC, ESTATE  # noqa: F401
 from . import sharding  # noqa: F401

@@ -25,8 +25,10 @@ EXPORTED_SYMBOLS = [
     "caspar_ba_export", "caspar_ba_schur_matvec", "caspar_ba_get_stats", "caspar_ba_set_profiling",
     "caspar_ba_last_error", "caspar_ba_layout_create", "caspar_ba_layout_get_info", "caspar_ba_layout_copy",
     "caspar_ba_layout_destroy", "caspar_ba_set_preconditioner", "caspar_ba_pcgnr_solve", "caspar_ba_set_linear_solver",
-    "caspar_ba_set_fusion", "caspar_ba_set_shard",
+    "caspar_ba_set_fusion", "caspar_ba_set_shard", "caspar_ba_cost_static",
 ]
+
+STATIC_MAX_CAMERAS = 16384  # CASPAR_BA_STATIC_MAX_CAMERAS
 
 
 class Problem(C.Structure):
@@ -136,6 +138,7 @@ def load_library() -> C.CDLL:
     L.caspar_ba_set_fusion.argtypes = [vp, C.c_int32]
     L.caspar_ba_set_shard.argtypes = [vp, EXCHANGE_FN, vp, vp, C.c_size_t, C.c_int32]
     L.caspar_ba_set_linear_solver.argtypes = [vp, C.c_int32]
+    L.caspar_ba_cost_static.argtypes = [C.POINTER(Problem), vp, vp]
     L.caspar_ba_pcgnr_solve.argtypes = [vp, C.c_float, C.c_float, C.c_int32, vp, C.POINTER(PcgInfo)]
     _lib = L
     return L
@@ -177,6 +180,32 @@ def plan_layout(num_cameras: int, num_points: int, camera_index, point_index, ti
 def _stream_ptr(stream: Optional[torch.cuda.Stream], device=None) -> int:
     """cudaStream_t of `stream`, default: the current stream OF `device` (not of whatever device is current)."""
     return (stream or torch.cuda.current_stream(device)).cuda_stream
+
+
+def cost_static(cameras: torch.Tensor, points: torch.Tensor, observations: torch.Tensor, camera_index: torch.Tensor,
+                point_index: torch.Tensor, cost_out: torch.Tensor, robust_loss: int = 0, robust_scale: float = 0.0,
+                depth_epsilon: float = 0.0, stream=None) -> None:
+    """caspar_ba_cost_static: F at the given parameters into `cost_out[0]` (CUDA float64), no handle, no allocation
+    (the library's fixed scratch array; at most STATIC_MAX_CAMERAS cameras).  Asynchronous on `stream`.  Every tensor
+    must already be a contiguous CUDA tensor of the right dtype: nothing is converted or copied here."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("caspar_ba needs a CUDA device; there is no CPU fallback")
+    for name, t, dtype in (("cameras", cameras, torch.float32), ("points", points, torch.float32),
+                           ("observations", observations, torch.float32), ("camera_index", camera_index, torch.int32),
+                           ("point_index", point_index, torch.int32), ("cost_out", cost_out, torch.float64)):
+        if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of dtype {dtype}")
+    if cost_out.numel() < 1 or camera_index.numel() != point_index.numel() or observations.numel() != 2 * camera_index.numel():
+        raise ValueError("cost_out needs one element; the index arrays one entry per observation")
+    L = load_library()
+    dev = cameras.device
+    pb = Problem(cameras.numel() // 9, points.numel() // 3, camera_index.numel(), cameras.data_ptr(),
+                 points.data_ptr(), observations.data_ptr(), camera_index.data_ptr(), point_index.data_ptr(),
+                 int(robust_loss), float(robust_scale), 0, 0, float(depth_epsilon))
+    with torch.cuda.device(dev):   # the entry point runs on the CURRENT device
+        rc = L.caspar_ba_cost_static(C.byref(pb), cost_out.data_ptr(), _stream_ptr(stream, dev))
+    if rc:
+        raise CasparError(rc, "cost_static", L.caspar_ba_last_error(None).decode())
 
 
 class CasparBA:

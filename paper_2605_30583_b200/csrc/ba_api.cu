@@ -694,6 +694,50 @@ int caspar_ba_cost(caspar_ba_t* h, void* cuda_stream, double* cost_out) {
   return std::isfinite(*cost_out) ? CASPAR_BA_OK : fail(h, CASPAR_BA_ENUMERIC, "non-finite cost");
 }
 
+// S9 without a handle and without an allocation: the scratch is the fixed device array of ba_kernels.cu.  The success
+// path touches no allocator (host or device); only a failure builds an error string.
+int caspar_ba_cost_static(const caspar_ba_problem* pb, double* cost_out_dev, void* cuda_stream) {
+  if (!pb || !cost_out_dev) return create_fail(CASPAR_BA_EINVAL, "null problem / cost_out_dev");
+  if (pb->num_cameras < 0 || pb->num_points < 0 || pb->num_observations < 0)
+    return create_fail(CASPAR_BA_EINVAL, "negative size");
+  if (pb->num_cameras > CASPAR_BA_STATIC_MAX_CAMERAS)
+    return create_fail(CASPAR_BA_EINVAL, "caspar_ba_cost_static: " + std::to_string(pb->num_cameras) +
+                                             " cameras exceed CASPAR_BA_STATIC_MAX_CAMERAS = " +
+                                             std::to_string(CASPAR_BA_STATIC_MAX_CAMERAS) +
+                                             " (the fixed scratch array holds one 144-byte table row per camera)");
+  if (pb->num_observations > 0 && (!pb->observations || !pb->camera_index || !pb->point_index))
+    return create_fail(CASPAR_BA_EINVAL, "null observation / index array");
+  if ((pb->num_cameras > 0 && !pb->cameras) || (pb->num_points > 0 && !pb->points))
+    return create_fail(CASPAR_BA_EINVAL, "null parameter array");
+  if (pb->robust_loss != 0 && pb->robust_loss != 1) return create_fail(CASPAR_BA_EINVAL, "robust_loss must be 0 or 1");
+  if (pb->robust_loss == 1 && !(pb->robust_scale > 0.f))
+    return create_fail(CASPAR_BA_EINVAL, "robust_scale must be positive with the Cauchy loss");
+  if (!(pb->depth_epsilon >= 0.f)) return create_fail(CASPAR_BA_EINVAL, "depth_epsilon must be >= 0");
+  int device = -1;
+  cudaError_t e = cudaGetDevice(&device);
+  if (e != cudaSuccess) return create_fail(CASPAR_BA_ECUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+  // the kernels dereference every pointer on the current device: a host pointer would fault there
+  const void* ptrs[] = {pb->cameras, pb->points, pb->observations, pb->camera_index, pb->point_index, cost_out_dev};
+  const char* names[] = {"cameras", "points", "observations", "camera_index", "point_index", "cost_out_dev"};
+  for (int i = 0; i < 6; ++i) {
+    if (!ptrs[i]) continue;
+    cudaPointerAttributes a;
+    const bool ok = cudaPointerGetAttributes(&a, ptrs[i]) == cudaSuccess &&
+                    (a.type == cudaMemoryTypeManaged || (a.type == cudaMemoryTypeDevice && a.device == device));
+    if (!ok) {
+      cudaGetLastError();
+      return create_fail(CASPAR_BA_EINVAL, std::string("caspar_ba_cost_static: ") + names[i] +
+                                               " is not device memory of the current device");
+    }
+  }
+  e = launch_cost_static(pb->num_cameras, pb->num_points, pb->num_observations, pb->cameras, pb->points,
+                         pb->observations, pb->camera_index, pb->point_index, pb->robust_loss, pb->robust_scale,
+                         pb->depth_epsilon, cost_out_dev, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess)
+    return create_fail(CASPAR_BA_ECUDA, std::string("caspar_ba_cost_static: ") + cudaGetErrorString(e));
+  return CASPAR_BA_OK;
+}
+
 int caspar_ba_pcg_solve(caspar_ba_t* h, float lambda, float rel_tol, int32_t max_iter, void* cuda_stream,
                         caspar_ba_pcg_info* info) {
   if (!h || max_iter < 0 || !(lambda >= 0.f) || !(rel_tol >= 0.f)) return CASPAR_BA_EINVAL;

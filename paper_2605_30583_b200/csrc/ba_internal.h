@@ -215,5 +215,9 @@ cudaError_t launch_commit(const View& v, cudaStream_t s);
 cudaError_t launch_export(const View& v, int what, double* dst, cudaStream_t s);
 // `stage` (sharded handles): 0 = all, 1 = load + pass (leaves the shard's partial in v.q), 2 = finish (adds lambda D p)
 cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* q_out, cudaStream_t s, int stage = 0);
+// caspar_ba_cost_static: S1 + S9 on the caller's arrays with the scratch in a file-scope device array (no allocation)
+cudaError_t launch_cost_static(int nc, int np, long long n, const float* cameras, const float* points,
+                               const float* observations, const int* cam_idx, const int* pt_idx, int robust,
+                               float robust_scale, float depth_eps, double* cost_out, cudaStream_t s);
 
 }  // namespace cba

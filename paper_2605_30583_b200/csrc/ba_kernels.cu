@@ -16,6 +16,7 @@
 #include <math_constants.h>
 
 #include <cstdlib>
+#include <mutex>
 
 #include "ba_internal.h"
 
@@ -2445,6 +2446,114 @@ cudaError_t launch_matvec_standalone(const View& v, const double* p_in, double* 
   if (e != cudaSuccess || stage == 1) return e;
   matvec_finish_kernel<<<g, 256, 0, s>>>(v, q_out);
   return CBA_LAUNCHED();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Allocation-free cost (caspar_ba_cost_static; include/caspar_ba.h): step S9 on the CALLER's arrays, without a
+// handle and without any cudaMalloc.  The scratch the handle path keeps in its arena (the S1 camera table and the
+// per-block cost partials) lives in ONE file-scope device array of a fixed size.
+//
+// Every device that loads the library holds these kStaticScratchBytes until the process exits.  All calls share the
+// array: calls that overlap on one GPU (two streams, two threads) race on it.  Nothing in it has to start at zero:
+// every word a call reads -- table rows [0, nc), partials [0, kStaticCostBlocks) -- that call has written first, so
+// the previous call's contents never show.
+//
+// `g_static_scratch` is a device symbol: in host code its name is only a host-side stand-in, NOT a device address.
+// The launcher asks the runtime for the address once per device (cudaGetSymbolAddress, that device current) and
+// hands the kernels that pointer.
+// ------------------------------------------------------------------------------------------------
+constexpr int kStaticCostBlocks = 148 * 4;
+constexpr int kStaticCostThreads = 256;
+constexpr size_t kStaticTableBytes = (size_t)CASPAR_BA_STATIC_MAX_CAMERAS * kCamTableFloats * sizeof(float);
+constexpr size_t kStaticScratchBytes = kStaticTableBytes + kStaticCostBlocks * sizeof(double);
+static_assert(kStaticTableBytes % 256 == 0, "the partials start on a 256-byte boundary");
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+// One thread per observation (grid-stride, caller's order): the same fp64 residual as the S9 kernels
+// (residual_observation, loss_term), summed per thread, then per block in a fixed tree; part[block] is always
+// written.  An index out of range poisons the sum (NaN) instead of faulting.
+__global__ void __launch_bounds__(kStaticCostThreads)
+cost_static_kernel(View v, const float* __restrict__ table, const float* __restrict__ points,
+                   const float2* __restrict__ observations, const int* __restrict__ cam_idx,
+                   const int* __restrict__ pt_idx, long long n, double* __restrict__ part) {
+  __shared__ double red[32];
+  double acc = 0.0;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const int c = __ldg(cam_idx + i), k = __ldg(pt_idx + i);
+    if (c < 0 || c >= v.nc || k < 0 || k >= v.np) {
+      acc += __longlong_as_double(0x7ff8000000000000ll);
+      continue;
+    }
+    const float* X = points + 3ll * k;
+    double r0, r1;
+    residual_observation(table, c, __ldg(X), __ldg(X + 1), __ldg(X + 2), __ldg(observations + i), v.depth_eps, r0, r1);
+    acc += loss_term(v, fma(r0, r0, r1 * r1)).rho;
+  }
+  const double tot = block_sum(acc, red);
+  if (threadIdx.x == 0) part[blockIdx.x] = tot;
+}
+
+// F = 1/2 sum of the block partials, in block order (bitwise reproducible for a given input).
+__global__ void __launch_bounds__(1024) cost_static_finish_kernel(const double* __restrict__ part, int n,
+                                                                 double* __restrict__ out) {
+  __shared__ double red[32];
+  double a = 0.0;
+  for (int i = threadIdx.x; i < n; i += 1024) a += part[i];
+  const double tot = block_sum(a, red);
+  if (threadIdx.x == 0) *out = 0.5 * tot;
+}
+
+// Device address of g_static_scratch on the CURRENT device, looked up once per device.
+static cudaError_t static_scratch_address(unsigned char** out) {
+  constexpr int kMaxDevices = 64;
+  static std::mutex mu;
+  static unsigned char* address[kMaxDevices] = {};
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!address[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    address[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = address[dev];
+  return cudaSuccess;
+}
+
+cudaError_t launch_cost_static(int nc, int np, long long n, const float* cameras, const float* points,
+                               const float* observations, const int* cam_idx, const int* pt_idx, int robust,
+                               float robust_scale, float depth_eps, double* cost_out, cudaStream_t s) {
+  if (nc > CASPAR_BA_STATIC_MAX_CAMERAS) return cudaErrorInvalidValue;
+  unsigned char* scratch = nullptr;
+  cudaError_t e = static_scratch_address(&scratch);
+  if (e != cudaSuccess) return e;
+  float* table = reinterpret_cast<float*>(scratch);
+  double* part = reinterpret_cast<double*>(scratch + kStaticTableBytes);
+  // (these launches are not counted into any handle's kernels_launched)
+  View v{};  // only the fields the residual and the loss read
+  v.nc = nc;
+  v.np = np;
+  v.robust = robust;
+  v.robust_c2 = robust_scale * robust_scale;
+  v.robust_inv_c2 = robust ? 1.0 / ((double)robust_scale * (double)robust_scale) : 0.0;
+  v.depth_eps = depth_eps;
+  if (nc > 0) {
+    camera_prepass_kernel<<<grid_for(nc, 128), 128, 0, s>>>(nc, cameras, table);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  cost_static_kernel<<<kStaticCostBlocks, kStaticCostThreads, 0, s>>>(
+      v, table, points, reinterpret_cast<const float2*>(observations), cam_idx, pt_idx, n, part);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  cost_static_finish_kernel<<<1, 1024, 0, s>>>(part, kStaticCostBlocks, cost_out);
+  return cudaGetLastError();
 }
 
 }  // namespace cba
