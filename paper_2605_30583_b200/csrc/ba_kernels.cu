@@ -1115,6 +1115,7 @@ struct PipeLayout {  // byte offsets inside one stage / inside the dynamic share
   int stages, groups, tbuf, tbuf_bytes, sbuf, sbuf_bytes, scratch, hot, bars, total;
 };
 
+constexpr int kHotShift = 23;  // HOT kernels carry (hot index + 1) << 23 in a slot's camera id: needs nc < 2^23 (ba_reorder.cpp)
 constexpr int kWarpScratchBytes = 1328;  // per consumer warp: 9 x 33 floats of products + 32 camera ids (1,316 B)
 
 // NG consumer groups of T threads share the ring; each group owns a staging area for the point-side sums
@@ -1249,7 +1250,7 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
     const unsigned char* st = smem + (size_t)s * L.stage_bytes;
     const int npts = reinterpret_cast<const int*>(st + L.meta)[0];
     const unsigned short* pt_start = reinterpret_cast<const unsigned short*>(st + L.meta + 16);
-    const int cam = reinterpret_cast<const int*>(st + L.cam)[gt];
+    int cam = reinterpret_cast<const int*>(st + L.cam)[gt];
     const unsigned rp = reinterpret_cast<const unsigned short*>(st + L.rank)[gt];
     const unsigned rank = rp & 255u, pid = rp >> 8;
     // ---- phase A: u = J_c p_j, scatter J_p^T u to the point-major staging rows
@@ -1258,6 +1259,12 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
       const float4* pv = reinterpret_cast<const float4*>(v.p32) + 3ll * cam;
       pa = __ldg(pv); pb = __ldg(pv + 1); pc = __ldg(pv + 2);
     }
+    // HOT: the slot's hot index rides above bit 23 of its camera id from here on (sign, equality of neighbours and the
+    // scratch row keep working).  The lookup is issued HERE, two barriers ahead of the camera-side walk: inside the
+    // walk it was a chain of dependent L2-latency loads, one per segment end (the 28 KB of L1 left beside the ring
+    // hold neither the table nor the p rows): Skewed 0.696 ms per matvec, 0.441 with the walk's lookups and adds
+    // knocked out, 0.67-0.68 with either kind of add alone knocked out.
+    if (HOT && cam >= 0) cam |= ((int)__ldg(v.hot_of_cam + cam) + 1) << kHotShift;
     // The point elimination (t_k, s_k, e) is carried in fp64: its rounding error is cond(V'_k) eps |u|, and in
     // fp32 that exceeds the lambda-sized margin that keeps S positive definite once lambda <= 1e-4 (see
     // schur_pass_kernel).  u itself stays an fp32 dot product: an error du in u passes through the
@@ -1398,9 +1405,10 @@ __global__ void __launch_bounds__(NG * T + 32, 1) schur_matvec_pipelined_kernel(
         for (int i = 0; i < 11; ++i) {
           acc += val[i];
           if (endm & (1u << i)) {
-            const int cm = camrow[s0 + i];
-            if (cm >= 0) {
-              const int hot = HOT ? (int)__ldg(v.hot_of_cam + cm) : -1;
+            const int cmh = camrow[s0 + i];
+            if (cmh >= 0) {
+              const int hot = HOT ? (cmh >> kHotShift) - 1 : -1;
+              const int cm = HOT ? (cmh & ((1 << kHotShift) - 1)) : cmh;
               if (hot >= 0) atomicAdd(hot_acc + 9 * hot + k, (double)acc);
               else atomicAdd(qk + 9ll * cm, (double)acc);
             }

@@ -262,7 +262,7 @@ int reorder_observations(int nc, int np, long long n, const int* cam_idx, const 
   // accumulated per CTA in shared memory by the pipelined matvec; every other camera goes straight to L2.
   out->hot_of_cam.assign(nc > 0 ? nc : 1, -1);
   out->hot_list.clear();
-  if (nc > 0 && n > 0) {
+  if (nc > 0 && nc < (1 << 23) && n > 0) {  // (the HOT kernels carry the hot index above bit 23 of a camera id)
     const long long limit = std::max<long long>(8192, 4 * (n / nc));
     std::vector<std::pair<long long, int>> big;
     for (int c = 0; c < nc; ++c)
